@@ -1,0 +1,231 @@
+"""ctypes driver around oracle/tdse_oracle.c (TEST INFRASTRUCTURE -- see package docstring).
+
+No arithmetic of the method happens here beyond the coefficient definitions of PAPER.md:87
+(`coefficients`) and dtype rounding of inputs; every loop lives in the C file.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = [os.path.join(_HERE, "tdse_oracle.c"), os.path.join(_HERE, "tdse_oracle_step.inc")]
+_SO = os.path.join(_HERE, "_build", "liboracle_tdse.so")
+_LOCK = threading.Lock()
+_LIB = None
+
+PERIODIC, DIRICHLET = 0, 1
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (-O2 -ffp-contract=off -fopenmp). Returns the .so path."""
+    os.makedirs(os.path.dirname(_SO), exist_ok=True)
+    newest = max(os.path.getmtime(p) for p in _SRC)
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < newest:
+        tmp = _SO + ".tmp.%d" % os.getpid()
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c99", "-shared", "-fPIC",
+               "-o", tmp, _SRC[0], "-lm"]
+        subprocess.run(cmd, check=True, cwd=_HERE)
+        os.replace(tmp, _SO)
+    return _SO
+
+
+def lib():
+    global _LIB
+    with _LOCK:
+        if _LIB is None:
+            L = C.CDLL(build())
+            dp, fp, ip = C.POINTER(C.c_double), C.POINTER(C.c_float), C.POINTER(C.c_int)
+            L.oracle_max_threads.restype = C.c_int
+            L.oracle_set_threads.argtypes = [C.c_int]
+            L.oracle_potential.argtypes = [C.c_int] * 3 + [C.c_double] + [C.c_int] * 3 + \
+                [dp, C.c_int, C.c_double, C.c_double, C.c_double, dp]
+            L.oracle_mask.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, dp]
+            L.oracle_wavepacket.argtypes = [C.c_int] * 3 + [C.c_double] * 9 + [dp, dp]
+            L.oracle_stagger.argtypes = [C.c_int] * 6 + [C.c_double] * 4 + [dp, dp, dp, dp]
+            for sfx, rp in (("f64", dp), ("f32", fp)):
+                f = getattr(L, "oracle_step_" + sfx)
+                f.restype = C.c_int
+                f.argtypes = [C.c_int] * 6 + [C.c_double] * 4 + [rp, rp, rp, rp, C.c_int,
+                              C.POINTER(C.c_longlong), C.c_int, C.c_int, C.c_double,
+                              dp, dp, C.c_int, ip]
+                g = getattr(L, "oracle_norm_" + sfx)
+                g.restype = None
+                g.argtypes = [C.c_int] * 6 + [C.c_double] * 5 + [rp, rp, rp, rp, dp, dp]
+            _LIB = L
+    return _LIB
+
+
+def max_threads() -> int:
+    return int(lib().oracle_max_threads())
+
+
+def set_threads(n: int) -> None:
+    lib().oracle_set_threads(int(n))
+
+
+def _p(a: np.ndarray, ct):
+    return a.ctypes.data_as(C.POINTER(ct))
+
+
+def coefficients(dx: float, dt: float, mass: float, hbar: float,
+                 dy: Optional[float] = None, dz: Optional[float] = None) -> Tuple[float, float, float, float]:
+    """c_x = hbar dt/(2 m dx^2) (same for y, z), c_v = dt/hbar."""
+    dy = dx if dy is None else dy
+    dz = dx if dz is None else dz
+    return (hbar * dt / (2.0 * mass * dx * dx), hbar * dt / (2.0 * mass * dy * dy),
+            hbar * dt / (2.0 * mass * dz * dz), dt / hbar)
+
+
+def paper_time_step(dx: float, dy: float, dz: float, mass: float, hbar: float) -> float:
+    """eq (11): dt = (m / 5 hbar) min(dx, dy, dz)^2."""
+    return mass / (5.0 * hbar) * min(dx, dy, dz) ** 2
+
+
+def paper_wavelength(energy: float, mass: float, hbar: float) -> float:
+    """eq (4): lambda = sqrt(2 hbar^2 pi^2 / (m E))."""
+    return float(np.sqrt(2.0 * hbar * hbar * np.pi ** 2 / (mass * energy)))
+
+
+def potential(nx, ny, nz, dx, bc, atoms, vmin, vmax, rcut=0.0) -> np.ndarray:
+    atoms = np.ascontiguousarray(np.asarray(atoms, dtype=np.float64).reshape(-1, 6))
+    V = np.empty((nz, ny, nx), dtype=np.float64)
+    lib().oracle_potential(nx, ny, nz, dx, bc[0], bc[1], bc[2], _p(atoms, C.c_double),
+                           atoms.shape[0], vmin, vmax, rcut, _p(V, C.c_double))
+    return V
+
+
+def mask(nz, w_lo, w_hi, strength=0.05, power=2) -> np.ndarray:
+    M = np.empty(nz, dtype=np.float64)
+    lib().oracle_mask(nz, w_lo, w_hi, strength, power, _p(M, C.c_double))
+    return M
+
+
+def wavepacket(nx, ny, nz, dx, x0, y0, z0, sigma, kx, ky, kz, amplitude=0.0):
+    R0 = np.empty((nz, ny, nx), dtype=np.float64)
+    J0 = np.empty((nz, ny, nx), dtype=np.float64)
+    lib().oracle_wavepacket(nx, ny, nz, dx, x0, y0, z0, sigma, kx, ky, kz, amplitude,
+                            _p(R0, C.c_double), _p(J0, C.c_double))
+    return R0, J0
+
+
+def stagger(bc, coef, V, R0, J0) -> np.ndarray:
+    nz, ny, nx = R0.shape
+    V = np.ascontiguousarray(V, dtype=np.float64)
+    out = np.empty_like(R0)
+    lib().oracle_stagger(nx, ny, nz, bc[0], bc[1], bc[2], coef[0], coef[1], coef[2], coef[3],
+                         _p(V, C.c_double), _p(R0, C.c_double), _p(J0, C.c_double), _p(out, C.c_double))
+    return out
+
+
+class OracleRun:
+    """One batch entry of the hot path, step by step.
+
+    dtype: arithmetic type of the recurrence ("f64" | "f32").
+    round_to: if "f32" while dtype == "f64", every input (V, M, R0, I_half, coefficients) is
+    rounded to float and promoted back, so that the run is the exact-arithmetic image of an
+    fp32 run (used as the truth for fp32 parity).
+    """
+
+    def __init__(self, nx, ny, nz, dx, dt, mass=1.0, hbar=1.0, dtype="f64",
+                 bc=(DIRICHLET, DIRICHLET, DIRICHLET), absorb_lo=0, absorb_hi=0,
+                 strength=0.05, power=2, round_to: Optional[str] = None):
+        assert dtype in ("f64", "f32")
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.dx, self.dt, self.mass, self.hbar = float(dx), float(dt), float(mass), float(hbar)
+        self.dtype = dtype
+        self.np = np.float64 if dtype == "f64" else np.float32
+        self.round_to = round_to if round_to else dtype
+        self.bc = tuple(int(b) for b in bc)
+        coef = coefficients(dx, dt, mass, hbar)
+        self.coef = tuple(self._round_scalar(c) for c in coef)
+        self.M = self._round(mask(self.nz, absorb_lo, absorb_hi, strength, power))
+        self.V = None
+        self.R = None
+        self.I = None
+        self.k_det, self.every = 0, 0
+        self.D = np.zeros((self.ny, self.nx), dtype=np.float64)
+        self.trace = []
+        self.counter = C.c_longlong(0)
+
+    # -- rounding of inputs to the run's storage dtype --------------------------------
+    def _round(self, a: np.ndarray) -> np.ndarray:
+        a = np.asarray(a, dtype=np.float64)
+        if self.round_to == "f32":
+            a = a.astype(np.float32)
+        return np.ascontiguousarray(a.astype(self.np))
+
+    def _round_scalar(self, x: float) -> float:
+        return float(np.float32(x)) if self.round_to == "f32" else float(x)
+
+    # -- inputs ---------------------------------------------------------------------
+    def set_potential_atoms(self, atoms, vmin, vmax, rcut=0.0):
+        self.V64 = potential(self.nx, self.ny, self.nz, self.dx, self.bc, atoms, vmin, vmax, rcut)
+        self.V = self._round(self.V64)
+        return self
+
+    def set_potential_grid(self, V):
+        self.V64 = np.asarray(V, dtype=np.float64).reshape(self.nz, self.ny, self.nx)
+        self.V = self._round(self.V64)
+        return self
+
+    def set_wavepacket(self, x0, y0, z0, sigma, kx, ky, kz, amplitude=0.0):
+        assert self.V is not None, "potential first (the staggered start needs V)"
+        R0, J0 = wavepacket(self.nx, self.ny, self.nz, self.dx, x0, y0, z0, sigma, kx, ky, kz, amplitude)
+        Ih = stagger(self.bc, coefficients(self.dx, self.dt, self.mass, self.hbar),
+                     self.V.astype(np.float64), R0, J0)
+        self.R, self.I = self._round(R0), self._round(Ih)
+        self.counter = C.c_longlong(0)
+        return self
+
+    def set_state(self, R, I_half):
+        self.R = self._round(np.asarray(R).reshape(self.nz, self.ny, self.nx))
+        self.I = self._round(np.asarray(I_half).reshape(self.nz, self.ny, self.nx))
+        self.counter = C.c_longlong(0)
+        return self
+
+    def set_detector(self, k_plane, every):
+        self.k_det, self.every = int(k_plane), int(every)
+        self.D[:] = 0.0
+        self.trace = []
+        self.counter = C.c_longlong(0)
+        return self
+
+    # -- the recurrence -------------------------------------------------------------
+    def step(self, n: int):
+        assert self.V is not None and self.R is not None
+        ct = C.c_double if self.dtype == "f64" else C.c_float
+        f = getattr(lib(), "oracle_step_" + self.dtype)
+        cap = n // self.every + 2 if self.every > 0 else 1
+        tr = np.zeros(cap, dtype=np.float64)
+        ns = C.c_int(0)
+        f(self.nx, self.ny, self.nz, *self.bc, *self.coef,
+          _p(self.V, ct), _p(self.M, ct), _p(self.R, ct), _p(self.I, ct), int(n),
+          C.byref(self.counter), self.k_det, self.every, self.dx,
+          _p(self.D, C.c_double), _p(tr, C.c_double), cap, C.byref(ns))
+        self.trace.extend(tr[: ns.value].tolist())
+        return self
+
+    def norm(self) -> Tuple[float, float]:
+        ct = C.c_double if self.dtype == "f64" else C.c_float
+        g = getattr(lib(), "oracle_norm_" + self.dtype)
+        qv, qp = C.c_double(0), C.c_double(0)
+        g(self.nx, self.ny, self.nz, *self.bc, *self.coef, self.dx,
+          _p(self.V, ct), _p(self.M, ct), _p(self.R, ct), _p(self.I, ct), C.byref(qv), C.byref(qp))
+        return qv.value, qp.value
+
+    @classmethod
+    def from_workload(cls, w, entry: int = 0, dtype: Optional[str] = None,
+                      round_to: Optional[str] = None) -> "OracleRun":
+        """Set up batch entry `entry` of a workloads.Workload (inputs only; no stepping)."""
+        o = cls(w.nx, w.ny, w.nz, w.dx, w.dt, w.mass, w.hbar, dtype or w.dtype, w.bc,
+                w.absorb_lo, w.absorb_hi, w.strength, w.power, round_to=round_to)
+        o.set_potential_atoms(w.atoms[entry], w.vmin, w.vmax, w.rcut)
+        o.set_wavepacket(**w.packet)
+        o.set_detector(w.k_det, w.every)
+        return o
