@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the FDTD/TDSE hot path on B200 (contract: see DESIGN.md "Measurement").
+
+One bench "step" = one pass of the whole hot path over one batch of synthetic input:
+  S0 potential build for every entry, S1 packet init, S2-S4 `nsteps` fused FDTD steps with
+  boundary handling and absorber, S5 detector accumulation (+ trace), S6 all entries batched.
+Default workload: BASELINE.json configs[3] (64 x 128^3 fp32, 4000 steps) -- the configuration the
+metric's "trajectories/hour" is quoted on and the smallest one that streams from HBM rather than L2.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfgN]
+                  [--nsteps S] [--batch B]
+
+Prints ONE JSON line (rank 0).  `value` is whole-job Gcell-updates/s with inputs resident in HBM;
+`e2e` is the same through the C ABI with host buffers (atom lists H2D, detector images D2H).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+from workloads import make_config
+
+METRIC = "fdtd_gcell_updates_per_s"
+UNIT = "Gcell-updates/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--nsteps", type=int, default=0, help="FDTD steps per trajectory (0 = the config's)")
+    ap.add_argument("--batch", type=int, default=0, help="batch entries (0 = the config's)")
+    ap.add_argument("--dtype", default="", help="override dtype (cfg4: f32|f64)")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 two-pass, 2 fused")
+    ap.add_argument("--tblock", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload_from_args(a, rank=0):
+    idx = int(a.workload.replace("cfg", ""))
+    kw = {}
+    if a.batch:
+        kw["batch"] = a.batch
+    if a.dtype:
+        kw["dtype"] = a.dtype
+    w = make_config(idx, **kw)
+    if a.nsteps:
+        w = w.with_(steps=a.nsteps)
+    return idx, w
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
+
+
+def traffic_from_profiles(kernel_key: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu summary, or None."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 2 and f[0] == kernel_key:
+            try:
+                return float(f[1])
+            except ValueError:
+                return None
+    return None
+
+
+class ClockSampler:
+    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+             "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(prefix="clocks_", suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.gpu), "--query-gpu=" + self.QUERY, "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        try:
+            self.proc.terminate()
+            self.proc.wait(timeout=5)
+        except Exception:
+            try:
+                self.proc.kill()
+            except Exception:
+                pass
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                f = [x.strip() for x in line.split(",")]
+                if len(f) < 9:
+                    continue
+                try:
+                    sm.append(float(f[1])); mx.append(float(f[2]))
+                except ValueError:
+                    continue
+                for n, v in zip(names, f[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def run_reference(a):
+    """--impl reference: the CPU oracle as it stands, on the host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    idx, w = workload_from_args(a)
+    cores = oracle.max_threads()
+    nsample = 40 if w.cells <= 128 ** 3 else 4
+    o = oracle.OracleRun.from_workload(w, entry=0, dtype=w.dtype)
+    for _ in range(max(a.warmup, 0)):
+        o.step(nsample)
+    t0 = time.perf_counter()
+    for _ in range(a.steps):
+        o.step(nsample)
+    dt = time.perf_counter() - t0
+    val = w.cells * nsample * a.steps / dt / 1e9
+    sample = "entry 0 of %s, %d FDTD steps per bench step (of %d), potential and packet built once outside the timed region" % (
+        w.name, nsample, w.steps)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
+        "warmup": a.warmup, "ms_per_step": 1e3 * dt / max(a.steps, 1), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": w.dtype, "data": "synthetic",
+        "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "batch": 1, "fdtd_steps_per_step": nsample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(w):
+    import oracle
+    cores = oracle.max_threads()
+    o = oracle.OracleRun.from_workload(w, entry=0, dtype=w.dtype)
+    t0 = time.perf_counter(); o.step(4); probe = (time.perf_counter() - t0) / 4
+    n = int(max(4, min(w.steps, 12.0 / max(probe, 1e-6))))
+    t0 = time.perf_counter(); o.step(n); dt = time.perf_counter() - t0
+    return {"value": w.cells * n / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "entry 0 of %s, %d of %d FDTD steps (%.1f s)" % (w.name, n, w.steps, dt)}
+
+
+def main():
+    a = parse_args()
+    if a.impl == "reference":
+        return run_reference(a)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2401_07416_b200 import Tdse
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    idx, w = workload_from_args(a, rank)
+    if world > 1 and idx == 3:
+        # weak scaling: every rank generates its own 64 configurations (different seeds), no collective on the data path
+        from workloads.configs import _film_atoms, fcc111_slab
+        lx, ly, lz = w.nx * w.dx, w.ny * w.dx, w.nz * w.dx
+        slab = fcc111_slab(lx, ly, 0.55 * lz, 3)
+        atoms = []
+        for b in range(w.batch):
+            rng = np.random.default_rng(3000 + rank * w.batch + b)
+            atoms.append(np.concatenate([slab, _film_atoms(rng, lx, ly, 0.55 * lz, 12, 0.1, 0.5)], axis=0))
+        w = w.with_(atoms=atoms)
+
+    stream = torch.cuda.Stream()
+    t = Tdse(w.nx, w.ny, w.nz, w.batch, w.dx, w.dt, w.mass, w.hbar, w.dtype, stream=stream, device="cuda:%d" % local_rank)
+    t.set_boundary(*w.bc, w.absorb_lo, w.absorb_hi, w.strength, w.power)
+    t.set_option("kernel", a.kernel)
+    t.set_option("tblock", a.tblock)
+    max_samples = max(1, w.steps // max(w.every, 1))
+    p = w.packet
+    wbytes = 4 if w.dtype == "f32" else 8
+
+    # device-resident inputs for `value`; pinned host inputs for `e2e`
+    atoms_dev = [torch.from_numpy(np.ascontiguousarray(x)).to("cuda:%d" % local_rank) for x in w.atoms]
+    atoms_host = [np.ascontiguousarray(x) for x in w.atoms]
+    img_host = torch.empty((w.batch, w.ny, w.nx), dtype=torch.float64).pin_memory().numpy()
+    tr_host = np.zeros((w.batch, max_samples))
+    torch.cuda.synchronize()
+
+    def one_pass_device():
+        for b in range(w.batch):
+            t.set_potential_device(b, atoms_dev[b], w.atoms[b].shape[0], w.vmin, w.vmax, w.rcut)
+        t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
+        t.set_detector(w.k_det, w.every, max_samples)
+        t.step(w.steps)
+
+    import ctypes as C
+
+    def one_pass_host():
+        for b in range(w.batch):
+            t.set_potential(b, atoms_host[b], w.vmin, w.vmax, w.rcut)
+        t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
+        t.set_detector(w.k_det, w.every, max_samples)
+        t.step(w.steps)
+        ns = C.c_int(0)
+        dp = C.POINTER(C.c_double)
+        for b in range(w.batch):
+            t._check(t.L.tdse_detector_read(t._h, b, img_host[b].ctypes.data_as(dp), tr_host[b].ctypes.data_as(dp),
+                                            max_samples, C.byref(ns)), "tdse_detector_read")
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        v = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(v, op=dist.ReduceOp.MAX)
+        return float(v.item())
+
+    # ---- warm-up ---------------------------------------------------------------------------------
+    for _ in range(max(a.warmup, 0)):
+        one_pass_device()
+    barrier()
+
+    # ---- timed region: K passes, CUDA events on the launching stream -------------------------------
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    launches0 = t.get_info("launches")
+    step_ms = 0.0
+    barrier()
+    with torch.cuda.stream(stream):
+        ev[0].record(stream)
+        for _ in range(a.steps):
+            # S0, S1 then the step loop bracketed by its own events (dominant-kernel timing)
+            for b in range(w.batch):
+                t.set_potential_device(b, atoms_dev[b], w.atoms[b].shape[0], w.vmin, w.vmax, w.rcut)
+            t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
+            t.set_detector(w.k_det, w.every, max_samples)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            t.step(w.steps)
+            e1.record(stream)
+            ev.append((e0, e1))
+        ev[1].record(stream)
+    barrier()
+    total_ms = max_over_ranks(ev[0].elapsed_time(ev[1]))
+    for pair in ev[4:]:
+        step_ms += pair[0].elapsed_time(pair[1])
+    step_ms = max_over_ranks(step_ms)
+    launches = t.get_info("launches") - launches0
+    clocks = sampler.stop() if rank == 0 else {}
+    kernel, tblock = t.get_info("kernel"), t.get_info("tblock")
+
+    cell_updates = float(w.cells) * w.batch * w.steps * a.steps * world
+    value = cell_updates / (total_ms * 1e-3) / 1e9
+    step_value = cell_updates / (step_ms * 1e-3) / 1e9
+
+    # ---- e2e: host buffers through the C ABI, wall clock bracketed by synchronize + barrier ---------
+    e2e = None
+    if not a.no_e2e:
+        one_pass_host()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(a.steps):
+            one_pass_host()
+        torch.cuda.synchronize()
+        e2e_s = max_over_ranks(time.perf_counter() - t0)
+        h2d = sum(x.nbytes for x in atoms_host)
+        d2h = img_host.nbytes + tr_host.nbytes
+        e2e = {"value": cell_updates / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e2e_s / a.steps}
+
+    # ---- roofline of the dominant kernel (the FDTD step kernel) -------------------------------------
+    peak, peak_src, sm_max = peaks()
+    per_gpu_updates_per_launch = float(w.cells) * w.batch * max(tblock, 1)
+    nlaunch_step = (w.steps + max(tblock, 1) - 1) // max(tblock, 1) * a.steps if kernel == 2 else 2 * w.steps * a.steps
+    alg_bytes_per_launch = (5.0 * wbytes * per_gpu_updates_per_launch) if kernel == 2 else (4.0 * wbytes * float(w.cells) * w.batch)
+    avg_launch_s = (step_ms * 1e-3) / max(nlaunch_step, 1)
+    achieved = alg_bytes_per_launch / avg_launch_s / 1e9
+    kname = "fdtd_fused_T%d_%s" % (tblock, w.dtype) if kernel == 2 else "half_step_%s" % w.dtype
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": traffic_from_profiles(kname + "_" + a.workload), "kernel": kname, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes_per_launch, "avg_launch_ms": avg_launch_s * 1e3,
+                "step_loop_gcell_per_s": step_value,
+                "frac_of_8TBps_nominal": achieved / 8000.0}
+
+    if rank == 0:
+        cpu = None
+        if not a.no_cpu_baseline and world == 1:
+            cpu = cpu_baseline(w)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+            "ms_per_step": total_ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": w.dtype, "data": "synthetic",
+            "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "batch_per_gpu": w.batch, "fdtd_steps": w.steps,
+                       "parallelism": "batch entries sharded across GPUs, no collective" if world > 1 else "single GPU",
+                       "l2_policy": "working set %.1f GiB >> 126 MB L2 (inputs larger than L2, no flush needed)" % (
+                           5 * w.cells * w.batch * wbytes / 2 ** 30) if 5 * w.cells * w.batch * wbytes > 4 * 126e6
+                       else "working set fits L2: compulsory-basis roofline overstates DRAM traffic",
+                       "kernel": kname, "tile": [t.get_info("tile_x"), t.get_info("tile_y")], "z_chunks": t.get_info("z_chunks")},
+            "trajectories_per_hour": 3600.0 * w.batch * world * a.steps / (total_ms * 1e-3),
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+        }
+        print(json.dumps(line), flush=True)
+    t.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,175 @@
+/* tdse.h -- C ABI of libtdse: the FDTD leapfrog hot path of arXiv 2401.07416 on one B200.
+ *
+ * What the library computes (citations are /root/reference/PAPER.md line + equation):
+ *   - the split psi = psi_R + i psi_I on a rectangular mesh, eqs (5)-(7), PAPER.md:60-72;
+ *   - the leapfrog recurrence eq (9) (I half-step) then eq (8) (R half-step), PAPER.md:74-87,
+ *     with c = hbar dt / (2 m dx^2) and c_v = dt / hbar;
+ *   - periodic wrap of neighbour indices, eqs (13)-(14), or zero-Dirichlet faces;
+ *   - an absorbing layer (eq (10), realised as a multiplicative polynomial mask);
+ *   - the Gaussian packet of eq (3), started on the staggered time grid;
+ *   - the detector-plane density of eq (15), with the staggered density of PAPER.md:87;
+ *   - a synthetic potential summed from an atom list (BASELINE.json north_star (1)), which stands in for
+ *     the DFT potential of PAPER.md:50, 164.
+ * DESIGN.md lists every reading taken where the paper is silent or garbled.
+ *
+ * Conventions
+ *   - Every call returns an int status (TDSE_OK = 0, negative = error); nothing throws or aborts
+ *     across this boundary; out-parameters are written only on success; tdse_last_error() gives text.
+ *   - Layout: batch entry b, grid point (i, j, k) at position (i dx, j dx, k dx) lives at
+ *     flat offset ((b*nz + k)*ny + j)*nx + i, x fastest, in the context's dtype (float or double).
+ *     (The paper stores z fastest; this is a relabelling, reading 17.)
+ *   - "host" / "device" in a parameter name says where the pointer must live.  The caller owns every
+ *     buffer it passes in; the library copies atom lists before returning.  A workspace given to
+ *     tdse_bind() stays owned by the caller and must outlive the context.
+ *   - All work is enqueued on the stream given to tdse_bind() (default: the legacy null stream).
+ *     tdse_step() is asynchronous; calls that return data to the host synchronise that stream.
+ *   - One context is not thread-safe; distinct contexts are independent.
+ *   - There is no CPU fallback: every call needs a CUDA device and fails with TDSE_ECUDA without one.
+ */
+#ifndef TDSE_H
+#define TDSE_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tdse_ctx tdse_ctx;  /* opaque; created by tdse_create, freed by tdse_destroy */
+
+enum { TDSE_F32 = 0, TDSE_F64 = 1 };
+enum { TDSE_BC_PERIODIC = 0, TDSE_BC_DIRICHLET = 1 };  /* Dirichlet: values at index -1 and n are zero */
+enum {
+    TDSE_OK = 0,
+    TDSE_EINVAL = -1,     /* bad argument */
+    TDSE_ENOMEM = -2,     /* host or device allocation failed / workspace too small */
+    TDSE_ECUDA = -3,      /* CUDA runtime error (text in tdse_last_error) */
+    TDSE_ESTATE = -4,     /* call out of order (e.g. step before potential and state are set) */
+    TDSE_EUNSTABLE = -5   /* dt above the sufficient stability bound, see tdse_step */
+};
+
+/* One atom of the synthetic potential.  screen <= 0 (or non-finite) means "unscreened". */
+typedef struct { double x, y, z, Z, soft2, screen; } tdse_atom;
+
+/* Kernel variants selectable with tdse_set_option("kernel", v). */
+enum {
+    TDSE_KERNEL_AUTO = 0,     /* fused where the shape allows it, else two-pass */
+    TDSE_KERNEL_TWOPASS = 1,  /* one thread per cell, eq (9) launch then eq (8) launch, in place */
+    TDSE_KERNEL_FUSED = 2     /* z-marching fused R+I kernel, T full steps per pass (needs ping-pong) */
+};
+
+/* Create a context for `batch` independent nx*ny*nz grids with cubic cells of edge dx, time step dt,
+ * particle mass `mass`, reduced Planck constant `hbar`, arithmetic/storage type `dtype`.
+ * Defaults: periodic on all three axes, no absorber, detector off.
+ * Errors: TDSE_EINVAL (sizes < 1, non-positive dx/dt/mass/hbar, unknown dtype), TDSE_ECUDA, TDSE_ENOMEM. */
+int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
+                double dx, double dt, double mass, double hbar, int dtype);
+
+/* Free the context and everything the library allocated.  NULL is accepted. */
+int tdse_destroy(tdse_ctx* ctx);
+
+/* Bytes of device workspace for the R, I, V grids (pingpong = 0: 3 arrays, two-pass kernels only;
+ * pingpong = 1: 5 arrays, needed by the fused kernels).  Returns 0 on invalid arguments. */
+size_t tdse_workspace_bytes(int nx, int ny, int nz, int batch, int dtype, int pingpong);
+
+/* Use caller-owned device memory (e.g. a torch tensor) and a caller-owned CUDA stream (a cudaStream_t
+ * passed as void*; NULL = legacy default stream).  `bytes` >= tdse_workspace_bytes(..., 0); if it is
+ * also >= tdse_workspace_bytes(..., 1) the fused kernels become available.  dev_workspace must be
+ * 256-byte aligned.  If tdse_bind is never called the library allocates its own 5-array workspace on
+ * first use.  Rebinding discards potential and state.  Errors: TDSE_EINVAL, TDSE_ENOMEM. */
+int tdse_bind(tdse_ctx* ctx, void* dev_workspace, size_t bytes, void* cuda_stream);
+
+/* Boundary condition per axis and the absorbing layers at the two z faces.
+ * The freshly updated field is multiplied by M[k] after each half-step, with
+ *   M[k] = 1 - strength * xi^power,  xi = (absorb_lo - k)/absorb_lo  for k < absorb_lo,
+ *                                    xi = (k - (nz-1-absorb_hi))/absorb_hi  for k > nz-1-absorb_hi,
+ * M = 1 elsewhere; 0 cells = that layer is off.  Errors: TDSE_EINVAL (unknown bc, negative widths,
+ * absorb_lo + absorb_hi > nz, strength outside [0, 1], power < 1). */
+int tdse_set_boundary(tdse_ctx* ctx, int bcx, int bcy, int bcz,
+                      int absorb_lo, int absorb_hi, double strength, int power);
+
+/* Build V for entry b (b = -1: all entries) on the device from `natoms` atoms in HOST memory:
+ *   V = min(max( sum_a -Z_a * exp(-r_a/screen_a) / sqrt(r_a^2 + soft2_a), vmin), vmax)
+ * r_a = distance from the grid point to atom a, nearest periodic image on periodic axes, true distance
+ * on Dirichlet axes; rcut > 0 skips atoms with r_a > rcut.  Accumulated in double in list order and
+ * rounded once to the context dtype.  Uses the boundary flags in force at the time of the call.
+ * Errors: TDSE_EINVAL (b out of range, natoms < 0, NULL with natoms > 0, vmin > vmax), TDSE_ECUDA. */
+int tdse_set_potential(tdse_ctx* ctx, int b, const tdse_atom* atoms_host, int natoms,
+                       double vmin, double vmax, double rcut);
+
+/* Same, with the atom list already in DEVICE memory (must stay valid until the stream reaches the
+ * build kernel; the library does not copy it). */
+int tdse_set_potential_device(tdse_ctx* ctx, int b, const tdse_atom* atoms_device, int natoms,
+                              double vmin, double vmax, double rcut);
+
+/* Raw potential grid for entry b (b = -1: the same grid for all entries), nx*ny*nz values of the
+ * context dtype, layout [z][y][x]; on_device says where V lives (a gridded V). */
+int tdse_set_potential_grid(tdse_ctx* ctx, int b, const void* V, int on_device);
+
+/* Gaussian packet, eq (3) PAPER.md:52 with a signed wave vector:
+ *   psi0 = A exp(-|r - r0|^2 / (2 sigma^2)) exp(+i k.(r - r0)),  A = amplitude, or (pi sigma^2)^(-3/4)
+ * when amplitude == 0.  The paper's case is k = (0, 0, -2 pi / lambda), eq (4).  Stores
+ *   R^0 = Re psi0,   I^{-1/2} = Im psi0 + (1/2) (dt/hbar) (H Re psi0)
+ * (staggered start, reading 4), evaluated in double from the stored V and rounded once.
+ * Resets the step counter and the detector.  b = -1: all entries.
+ * Errors: TDSE_ESTATE (potential of that entry not set), TDSE_EINVAL (sigma <= 0, b out of range). */
+int tdse_set_wavepacket(tdse_ctx* ctx, int b, double x0, double y0, double z0, double sigma,
+                        double kx, double ky, double kz, double amplitude);
+
+/* Raw state for entry b (b = -1: the same state for all entries): R^n and I^{n-1/2}, nx*ny*nz values
+ * each of the context dtype, [z][y][x].  Resets the step counter and the detector. */
+int tdse_set_state(tdse_ctx* ctx, int b, const void* R, const void* I_half, int on_device);
+
+/* Detector plane k_plane (0 <= k_plane < nz), sampled after every `every`-th full step counted from the
+ * last reset (eq (15), h = `every`); every = 0 switches it off.  Each sample adds
+ *   rho(i,j) = R^s(i,j,k)^2 + I^{s-1/2}(i,j,k)^2      (density of PAPER.md:87)
+ * to a per-entry image (double) and appends dx^2 * sum_ij rho to a per-entry trace.  Resets image,
+ * trace and step counter.  `max_samples` traces are kept per entry (further samples still accumulate
+ * into the image but are not recorded in the trace).  Errors: TDSE_EINVAL. */
+int tdse_set_detector(tdse_ctx* ctx, int k_plane, int every, int max_samples);
+
+/* Advance every entry by n full time steps (eq (9) then eq (8), mask, detector), asynchronously on the
+ * bound stream.  Errors: TDSE_ESTATE if any entry lacks potential or state; TDSE_EUNSTABLE if
+ * dt > 2 hbar / (12 hbar^2 / (2 m dx^2) + max|V|) (sufficient bound for max|eig(dt H / hbar)| < 2;
+ * max|V| is taken over the clamp limits / raw grids seen so far), unless option "allow_unstable" is 1. */
+int tdse_step(tdse_ctx* ctx, int n);
+
+/* Copy entry b's accumulated detector image (ny*nx doubles, [y][x]) and the first min(cap, nsamples)
+ * trace values to HOST memory; *nsamples = samples taken so far.  NULL pointers skip that output.
+ * Synchronises the stream. */
+int tdse_detector_read(tdse_ctx* ctx, int b, double* image_host, double* trace_host, int cap, int* nsamples);
+
+/* Device pointers to the detector image [batch][ny][nx] and trace [batch][max_samples] (doubles);
+ * valid until the next tdse_set_detector or tdse_destroy.  Does not synchronise. */
+int tdse_detector_device(tdse_ctx* ctx, double** image_device, double** trace_device, int* max_samples);
+
+/* Copy entry b's R^n and I^{n-1/2} ([z][y][x], context dtype) to HOST memory. Synchronises. */
+int tdse_read_psi(tdse_ctx* ctx, int b, void* R_host, void* I_host);
+
+/* Copy entry b's potential ([z][y][x], context dtype) to HOST memory. Synchronises. */
+int tdse_read_potential(tdse_ctx* ctx, int b, void* V_host);
+
+/* Diagnostics for entry b, accumulated in double:
+ *   q_paper    = dx^3 sum (R^n)^2 + (I^{n-1/2})^2
+ *   q_visscher = dx^3 sum (R^n)^2 + I^{n+1/2} I^{n-1/2}         (conserved exactly when M == 1)
+ * I^{n+1/2} is one look-ahead eq (9) half-step (with mask) evaluated in double; state is not modified.
+ * Either pointer may be NULL.  Synchronises. */
+int tdse_norm(tdse_ctx* ctx, int b, double* q_visscher, double* q_paper);
+
+/* Options: "kernel" (TDSE_KERNEL_*), "tblock" (full steps fused per pass, 0 = auto, 1..2),
+ * "allow_unstable" (0/1).  Errors: TDSE_EINVAL for unknown keys or values. */
+int tdse_set_option(tdse_ctx* ctx, const char* key, long long value);
+
+/* Introspection: "launches" (kernels launched by this context so far), "steps" (full steps since the last
+ * reset), "kernel" / "tblock" (what tdse_step used last), "pingpong" (1 if 5-array workspace),
+ * "tile_x", "tile_y", "z_chunks" (fused launch shape used last).  Errors: TDSE_EINVAL. */
+int tdse_get_info(const tdse_ctx* ctx, const char* key, long long* value);
+
+/* Text of the last error on this context ("" if none).  Never NULL.  ctx may be NULL (global slot used
+ * by tdse_create failures). */
+const char* tdse_last_error(const tdse_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDSE_H */

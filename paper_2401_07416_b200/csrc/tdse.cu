@@ -1,0 +1,717 @@
+// tdse.cu -- C-ABI of libtdse (include/tdse.h): context, host-side scheduling, kernel launches.
+// sm_100a only.  No CPU fallback: every entry point fails with TDSE_ECUDA without a device.
+#include "../../include/tdse.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "tdse_common.cuh"
+#include "tdse_kernels_basic.cuh"
+#include "tdse_kernels_fused.cuh"
+
+using namespace tdse;
+
+namespace {
+
+std::string g_create_error;
+
+constexpr size_t kAlign = 256;
+inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+}  // namespace
+
+struct tdse_ctx {
+    Grid g{};
+    int dtype = TDSE_F64;
+    size_t w = 8;                       // bytes per element
+    double dx = 0, dt = 0, mass = 0, hbar = 0;
+    double c = 0, cv = 0;
+    int absorb_lo = 0, absorb_hi = 0, power = 2;
+    double strength = 0.0;
+
+    // workspace
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    bool ws_owned = false;
+    bool pingpong = false;
+    size_t arr_bytes = 0;               // aligned bytes of one [batch][nz][ny][nx] array
+    void* R[2] = {nullptr, nullptr};
+    void* I[2] = {nullptr, nullptr};
+    void* V = nullptr;
+    int cur = 0;
+    cudaStream_t stream = nullptr;
+
+    // small library-owned buffers
+    void* mask_dev = nullptr;           // real[nz]
+    std::vector<double> mask_host;
+    double* D = nullptr;                // [batch][ny][nx]
+    double* trace = nullptr;            // [batch][max_samples]
+    double* partial = nullptr;          // scratch for reductions
+    size_t partial_n = 0;
+    double* scalars = nullptr;          // 4 doubles
+    AtomRec* atoms_dev = nullptr;
+    AtomRec* atoms_pin = nullptr;
+    int atoms_cap = 0;
+    cudaEvent_t atoms_ev = nullptr;
+    bool atoms_pending = false;
+
+    int k_det = 0, every = 0, max_samples = 0, nsamples = 0;
+    long long steps = 0;
+    std::vector<char> have_V, have_state;
+    double vabs_max = 0.0;
+
+    // options / info
+    int opt_kernel = TDSE_KERNEL_AUTO, opt_tblock = 0, allow_unstable = 0;
+    long long launches = 0;
+    int last_kernel = 0, last_tblock = 0, last_tile_x = 0, last_tile_y = 0, last_chunks = 0;
+    int num_sms = 148;
+    std::string err;
+};
+
+namespace {
+
+int fail(tdse_ctx* ctx, int code, const std::string& msg)
+{
+    if (ctx) ctx->err = msg; else g_create_error = msg;
+    return code;
+}
+
+#define CU_TRY(ctx, expr)                                                                     \
+    do {                                                                                      \
+        cudaError_t e__ = (expr);                                                             \
+        if (e__ != cudaSuccess)                                                               \
+            return fail(ctx, TDSE_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e__)); \
+    } while (0)
+
+#define CU_LAUNCH_CHECK(ctx)                                                                     \
+    do {                                                                                         \
+        cudaError_t e__ = cudaGetLastError();                                                    \
+        if (e__ != cudaSuccess)                                                                  \
+            return fail(ctx, TDSE_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(e__)); \
+        ctx->launches++;                                                                         \
+    } while (0)
+
+inline size_t elem_bytes(int dtype) { return dtype == TDSE_F32 ? 4 : 8; }
+
+void carve(tdse_ctx* c)
+{
+    char* base = static_cast<char*>(c->ws);
+    c->R[0] = base;
+    c->I[0] = base + c->arr_bytes;
+    c->V = base + 2 * c->arr_bytes;
+    if (c->pingpong) {
+        c->R[1] = base + 3 * c->arr_bytes;
+        c->I[1] = base + 4 * c->arr_bytes;
+    } else {
+        c->R[1] = c->I[1] = nullptr;
+    }
+    c->cur = 0;
+    std::fill(c->have_V.begin(), c->have_V.end(), 0);
+    std::fill(c->have_state.begin(), c->have_state.end(), 0);
+    c->vabs_max = 0.0;
+}
+
+int ensure_workspace(tdse_ctx* c)
+{
+    if (c->ws) return TDSE_OK;
+    const size_t bytes = 5 * c->arr_bytes;
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, TDSE_ENOMEM, std::string("cudaMalloc workspace: ") + cudaGetErrorString(e));
+    }
+    c->ws = p; c->ws_bytes = bytes; c->ws_owned = true; c->pingpong = true;
+    carve(c);
+    return TDSE_OK;
+}
+
+int ensure_partial(tdse_ctx* c, size_t n)
+{
+    if (n <= c->partial_n) return TDSE_OK;
+    if (c->partial) { cudaStreamSynchronize(c->stream); cudaFree(c->partial); c->partial = nullptr; c->partial_n = 0; }
+    CU_TRY(c, cudaMalloc(&c->partial, n * sizeof(double)));
+    c->partial_n = n;
+    return TDSE_OK;
+}
+
+// Absorbing mask of include/tdse.h (tdse_set_boundary), double on the host, rounded once to dtype.
+int upload_mask(tdse_ctx* c)
+{
+    const int nz = c->g.nz;
+    c->mask_host.assign(nz, 1.0);
+    for (int k = 0; k < nz; ++k) {
+        double xi = 0.0;
+        if (c->absorb_lo > 0 && k < c->absorb_lo) xi = double(c->absorb_lo - k) / double(c->absorb_lo);
+        if (c->absorb_hi > 0 && k > nz - 1 - c->absorb_hi) xi = double(k - (nz - 1 - c->absorb_hi)) / double(c->absorb_hi);
+        if (xi > 0.0) {
+            double p = 1.0;
+            for (int q = 0; q < c->power; ++q) p *= xi;
+            c->mask_host[k] = 1.0 - c->strength * p;
+        }
+    }
+    if (!c->mask_dev) CU_TRY(c, cudaMalloc(&c->mask_dev, (size_t)nz * c->w));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    if (c->dtype == TDSE_F32) {
+        std::vector<float> m(nz);
+        for (int k = 0; k < nz; ++k) m[k] = (float)c->mask_host[k];
+        CU_TRY(c, cudaMemcpy(c->mask_dev, m.data(), (size_t)nz * 4, cudaMemcpyHostToDevice));
+    } else {
+        CU_TRY(c, cudaMemcpy(c->mask_dev, c->mask_host.data(), (size_t)nz * 8, cudaMemcpyHostToDevice));
+    }
+    return TDSE_OK;
+}
+
+int reset_detector(tdse_ctx* c)
+{
+    c->steps = 0;
+    c->nsamples = 0;
+    if (c->D) {
+        const long long n = (long long)c->g.batch * c->g.plane;
+        fill_zero_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 4096), 256, 0, c->stream>>>(c->D, n);
+        CU_LAUNCH_CHECK(c);
+    }
+    if (c->trace && c->max_samples > 0) {
+        const long long n = (long long)c->g.batch * c->max_samples;
+        fill_zero_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 4096), 256, 0, c->stream>>>(c->trace, n);
+        CU_LAUNCH_CHECK(c);
+    }
+    return TDSE_OK;
+}
+
+inline char* entry_ptr(const tdse_ctx* c, void* arr, int b) { return static_cast<char*>(arr) + (size_t)b * c->g.cells * c->w; }
+
+bool entry_range(const tdse_ctx* c, int b, int* b0, int* b1)
+{
+    if (b == -1) { *b0 = 0; *b1 = c->g.batch; return true; }
+    if (b < 0 || b >= c->g.batch) return false;
+    *b0 = b; *b1 = b + 1;
+    return true;
+}
+
+// ---------------------------------------------------------------------------------------------
+// fused launch table
+// ---------------------------------------------------------------------------------------------
+template <typename real, int T, int BX, int BY, int NT, int PF>
+int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm)
+{
+    using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
+    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        CU_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM_BYTES));
+        attr_set = true;
+    }
+    P.tiles_x = (c->g.nx + BX - 1) / BX;
+    P.tiles_y = (c->g.ny + BY - 1) / BY;
+    const long long units = (long long)P.tiles_x * P.tiles_y * c->g.batch;
+    // choose the number of z chunks: minimise waves * (chunk length + halo planes)
+    const long long slots = (long long)c->num_sms * ctas_per_sm;
+    const int H = Tr::H;
+    int best_n = 1;
+    double best_cost = std::numeric_limits<double>::max();
+    const int max_chunks = std::max(1, c->g.nz / std::max(4 * H, 8));
+    for (int n = 1; n <= max_chunks; ++n) {
+        const int bz = (c->g.nz + n - 1) / n;
+        const int n_eff = (c->g.nz + bz - 1) / bz;
+        const long long waves = (units * n_eff + slots - 1) / slots;
+        const double cost = (double)waves * (bz + 2 * H + 3);   // +3: pipeline fill/launch overhead in plane units
+        if (cost < best_cost - 1e-9) { best_cost = cost; best_n = n_eff; }
+    }
+    P.bz = (c->g.nz + best_n - 1) / best_n;
+    P.nchunks = (c->g.nz + P.bz - 1) / P.bz;
+    const long long grid = units * P.nchunks;
+    if (grid > 0x7fffffffLL) return fail(c, TDSE_EINVAL, "fused grid too large");
+    kern<<<(unsigned)grid, NT, Tr::SMEM_BYTES, c->stream>>>(P);
+    CU_LAUNCH_CHECK(c);
+    c->last_tile_x = BX; c->last_tile_y = BY; c->last_chunks = P.nchunks;
+    return TDSE_OK;
+}
+
+int launch_fused(tdse_ctx* c, FusedParams& P, int T)
+{
+    if (c->dtype == TDSE_F32) {
+        if (T == 2) return launch_fused_cfg<float, 2, 64, 32, 384, 2>(c, P, 1);
+        return launch_fused_cfg<float, 1, 64, 32, 672, 2>(c, P, 1);
+    }
+    if (T == 2) return launch_fused_cfg<double, 2, 32, 32, 416, 1>(c, P, 1);
+    return launch_fused_cfg<double, 1, 32, 32, 352, 2>(c, P, 1);
+}
+
+bool fused_supported(const tdse_ctx* c)
+{
+    const int vw = (int)(16 / c->w);
+    return c->pingpong && (c->g.nx % vw == 0);
+}
+
+template <typename real>
+int launch_twopass_step(tdse_ctx* c)
+{
+    const dim3 grid((unsigned)((c->g.cells + 255) / 256), (unsigned)c->g.batch);
+    real* R = static_cast<real*>(c->R[c->cur]);
+    real* I = static_cast<real*>(c->I[c->cur]);
+    const real* V = static_cast<const real*>(c->V);
+    const real* M = static_cast<const real*>(c->mask_dev);
+    half_step_kernel<real><<<grid, 256, 0, c->stream>>>(c->g, (real)c->c, (real)c->cv, (real)1, V, M, R, I);
+    CU_LAUNCH_CHECK(c);
+    half_step_kernel<real><<<grid, 256, 0, c->stream>>>(c->g, (real)c->c, (real)c->cv, (real)-1, V, M, I, R);
+    CU_LAUNCH_CHECK(c);
+    return TDSE_OK;
+}
+
+int finish_trace(tdse_ctx* c, int nparts)
+{
+    trace_finish_kernel<<<(c->g.batch + 127) / 128, 128, 0, c->stream>>>(
+        c->partial, nparts, c->dx * c->dx, c->trace, c->max_samples, c->nsamples, c->g.batch);
+    CU_LAUNCH_CHECK(c);
+    c->nsamples++;
+    return TDSE_OK;
+}
+
+template <typename real>
+int sample_detector_twopass(tdse_ctx* c)
+{
+    const unsigned nblk = (unsigned)((c->g.plane + 255) / 256);
+    int rc = ensure_partial(c, (size_t)nblk * c->g.batch);
+    if (rc) return rc;
+    detector_accum_kernel<real><<<dim3(nblk, (unsigned)c->g.batch), 256, 0, c->stream>>>(
+        c->g, c->k_det, static_cast<const real*>(c->R[c->cur]), static_cast<const real*>(c->I[c->cur]), c->D, c->partial);
+    CU_LAUNCH_CHECK(c);
+    return finish_trace(c, (int)nblk);
+}
+
+}  // namespace
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+extern "C" {
+
+const char* tdse_last_error(const tdse_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+size_t tdse_workspace_bytes(int nx, int ny, int nz, int batch, int dtype, int pingpong)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || batch < 1 || (dtype != TDSE_F32 && dtype != TDSE_F64)) return 0;
+    const size_t arr = align_up((size_t)nx * ny * nz * batch * elem_bytes(dtype));
+    return (pingpong ? 5 : 3) * arr;
+}
+
+int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
+                double dx, double dt, double mass, double hbar, int dtype)
+{
+    if (!out) return fail(nullptr, TDSE_EINVAL, "tdse_create: out is NULL");
+    if (nx < 1 || ny < 1 || nz < 1 || batch < 1) return fail(nullptr, TDSE_EINVAL, "tdse_create: sizes must be >= 1");
+    if (!(dx > 0) || !(dt > 0) || !(mass > 0) || !(hbar > 0)) return fail(nullptr, TDSE_EINVAL, "tdse_create: dx, dt, mass, hbar must be > 0");
+    if (dtype != TDSE_F32 && dtype != TDSE_F64) return fail(nullptr, TDSE_EINVAL, "tdse_create: unknown dtype");
+    if ((long long)nx * ny > 0x3fffffffLL) return fail(nullptr, TDSE_EINVAL, "tdse_create: nx*ny too large");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, TDSE_ECUDA, std::string("tdse_create: no CUDA device (") + cudaGetErrorString(e) + "); libtdse has no CPU fallback");
+    }
+    tdse_ctx* c = new (std::nothrow) tdse_ctx();
+    if (!c) return fail(nullptr, TDSE_ENOMEM, "tdse_create: out of host memory");
+    c->g.nx = nx; c->g.ny = ny; c->g.nz = nz; c->g.batch = batch;
+    c->g.bcx = c->g.bcy = c->g.bcz = BC_PERIODIC;
+    c->g.plane = (long long)nx * ny;
+    c->g.cells = c->g.plane * nz;
+    c->dtype = dtype; c->w = elem_bytes(dtype);
+    c->dx = dx; c->dt = dt; c->mass = mass; c->hbar = hbar;
+    c->c = hbar * dt / (2.0 * mass * dx * dx);
+    c->cv = dt / hbar;
+    c->arr_bytes = align_up((size_t)c->g.cells * batch * c->w);
+    c->have_V.assign(batch, 0);
+    c->have_state.assign(batch, 0);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    auto bail = [&](const char* what, cudaError_t err) {
+        std::string m = std::string("tdse_create: ") + what + ": " + cudaGetErrorString(err);
+        tdse_destroy(c);
+        return fail(nullptr, TDSE_ECUDA, m);
+    };
+    if ((e = cudaMalloc(&c->D, (size_t)batch * c->g.plane * sizeof(double))) != cudaSuccess) return bail("detector image", e);
+    if ((e = cudaMalloc(&c->scalars, 4 * sizeof(double))) != cudaSuccess) return bail("scalars", e);
+    if ((e = cudaEventCreateWithFlags(&c->atoms_ev, cudaEventDisableTiming)) != cudaSuccess) return bail("event", e);
+    int rc = upload_mask(c);
+    if (rc) { std::string m = c->err; tdse_destroy(c); return fail(nullptr, rc, m); }
+    rc = reset_detector(c);
+    if (rc) { std::string m = c->err; tdse_destroy(c); return fail(nullptr, rc, m); }
+    *out = c;
+    return TDSE_OK;
+}
+
+int tdse_destroy(tdse_ctx* c)
+{
+    if (!c) return TDSE_OK;
+    cudaStreamSynchronize(c->stream);
+    if (c->ws_owned && c->ws) cudaFree(c->ws);
+    if (c->mask_dev) cudaFree(c->mask_dev);
+    if (c->D) cudaFree(c->D);
+    if (c->trace) cudaFree(c->trace);
+    if (c->partial) cudaFree(c->partial);
+    if (c->scalars) cudaFree(c->scalars);
+    if (c->atoms_dev) cudaFree(c->atoms_dev);
+    if (c->atoms_pin) cudaFreeHost(c->atoms_pin);
+    if (c->atoms_ev) cudaEventDestroy(c->atoms_ev);
+    cudaGetLastError();
+    delete c;
+    return TDSE_OK;
+}
+
+int tdse_bind(tdse_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream)
+{
+    if (!c) return TDSE_EINVAL;
+    if (!dev_workspace) return fail(c, TDSE_EINVAL, "tdse_bind: workspace is NULL");
+    if (reinterpret_cast<uintptr_t>(dev_workspace) % kAlign) return fail(c, TDSE_EINVAL, "tdse_bind: workspace must be 256-byte aligned");
+    if (bytes < 3 * c->arr_bytes) return fail(c, TDSE_ENOMEM, "tdse_bind: workspace smaller than tdse_workspace_bytes(..., 0)");
+    cudaStreamSynchronize(c->stream);
+    if (c->ws_owned && c->ws) cudaFree(c->ws);
+    c->ws = dev_workspace; c->ws_bytes = bytes; c->ws_owned = false;
+    c->pingpong = bytes >= 5 * c->arr_bytes;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    carve(c);
+    return reset_detector(c);
+}
+
+int tdse_set_boundary(tdse_ctx* c, int bcx, int bcy, int bcz, int absorb_lo, int absorb_hi, double strength, int power)
+{
+    if (!c) return TDSE_EINVAL;
+    auto okbc = [](int b) { return b == TDSE_BC_PERIODIC || b == TDSE_BC_DIRICHLET; };
+    if (!okbc(bcx) || !okbc(bcy) || !okbc(bcz)) return fail(c, TDSE_EINVAL, "tdse_set_boundary: unknown boundary flag");
+    if (absorb_lo < 0 || absorb_hi < 0 || absorb_lo + absorb_hi > c->g.nz) return fail(c, TDSE_EINVAL, "tdse_set_boundary: absorber widths");
+    if (!(strength >= 0.0 && strength <= 1.0) || power < 1) return fail(c, TDSE_EINVAL, "tdse_set_boundary: strength in [0,1], power >= 1");
+    c->g.bcx = bcx; c->g.bcy = bcy; c->g.bcz = bcz;
+    c->absorb_lo = absorb_lo; c->absorb_hi = absorb_hi; c->strength = strength; c->power = power;
+    return upload_mask(c);
+}
+
+static int build_potential(tdse_ctx* c, int b, const AtomRec* atoms_dev, int natoms, double vmin, double vmax, double rcut)
+{
+    int b0, b1;
+    if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_potential: entry out of range");
+    const unsigned nblk = (unsigned)((c->g.cells + 255) / 256);
+    void* dst = entry_ptr(c, c->V, b0);
+    if (c->dtype == TDSE_F32)
+        potential_build_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->dx, atoms_dev, natoms, vmin, vmax, rcut, static_cast<float*>(dst));
+    else
+        potential_build_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->dx, atoms_dev, natoms, vmin, vmax, rcut, static_cast<double*>(dst));
+    CU_LAUNCH_CHECK(c);
+    for (int e = b0 + 1; e < b1; ++e)
+        CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->V, e), dst, (size_t)c->g.cells * c->w, cudaMemcpyDeviceToDevice, c->stream));
+    for (int e = b0; e < b1; ++e) c->have_V[e] = 1;
+    c->vabs_max = std::max(c->vabs_max, std::max(std::fabs(vmin), std::fabs(vmax)));
+    return TDSE_OK;
+}
+
+int tdse_set_potential(tdse_ctx* c, int b, const tdse_atom* atoms_host, int natoms, double vmin, double vmax, double rcut)
+{
+    if (!c) return TDSE_EINVAL;
+    if (natoms < 0 || (natoms > 0 && !atoms_host)) return fail(c, TDSE_EINVAL, "tdse_set_potential: atom list");
+    if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential: vmin > vmax");
+    int rc = ensure_workspace(c);
+    if (rc) return rc;
+    if (natoms > c->atoms_cap) {
+        CU_TRY(c, cudaStreamSynchronize(c->stream));
+        if (c->atoms_dev) cudaFree(c->atoms_dev);
+        if (c->atoms_pin) cudaFreeHost(c->atoms_pin);
+        c->atoms_dev = nullptr; c->atoms_pin = nullptr; c->atoms_cap = 0;
+        const int cap = std::max(natoms, 1024);
+        CU_TRY(c, cudaMalloc(&c->atoms_dev, (size_t)cap * sizeof(AtomRec)));
+        CU_TRY(c, cudaMallocHost(&c->atoms_pin, (size_t)cap * sizeof(AtomRec)));
+        c->atoms_cap = cap;
+        c->atoms_pending = false;
+    }
+    if (c->atoms_pending) { CU_TRY(c, cudaEventSynchronize(c->atoms_ev)); c->atoms_pending = false; }
+    if (natoms > 0) {
+        static_assert(sizeof(AtomRec) == sizeof(tdse_atom), "atom record layout");
+        std::memcpy(c->atoms_pin, atoms_host, (size_t)natoms * sizeof(AtomRec));
+        CU_TRY(c, cudaMemcpyAsync(c->atoms_dev, c->atoms_pin, (size_t)natoms * sizeof(AtomRec), cudaMemcpyHostToDevice, c->stream));
+        // the pinned staging buffer may be rewritten once this copy is done (event); the device copy is
+        // rewritten by the next call's H2D, which the stream orders after this call's build kernel
+        CU_TRY(c, cudaEventRecord(c->atoms_ev, c->stream));
+        c->atoms_pending = true;
+    }
+    return build_potential(c, b, c->atoms_dev, natoms, vmin, vmax, rcut);
+}
+
+int tdse_set_potential_device(tdse_ctx* c, int b, const tdse_atom* atoms_device, int natoms, double vmin, double vmax, double rcut)
+{
+    if (!c) return TDSE_EINVAL;
+    if (natoms < 0 || (natoms > 0 && !atoms_device)) return fail(c, TDSE_EINVAL, "tdse_set_potential_device: atom list");
+    if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential_device: vmin > vmax");
+    int rc = ensure_workspace(c);
+    if (rc) return rc;
+    return build_potential(c, b, reinterpret_cast<const AtomRec*>(atoms_device), natoms, vmin, vmax, rcut);
+}
+
+int tdse_set_potential_grid(tdse_ctx* c, int b, const void* V, int on_device)
+{
+    if (!c) return TDSE_EINVAL;
+    if (!V) return fail(c, TDSE_EINVAL, "tdse_set_potential_grid: V is NULL");
+    int b0, b1;
+    if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_potential_grid: entry out of range");
+    int rc = ensure_workspace(c);
+    if (rc) return rc;
+    const size_t nbytes = (size_t)c->g.cells * c->w;
+    for (int e = b0; e < b1; ++e) {
+        CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->V, e), V, nbytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+        c->have_V[e] = 1;
+    }
+    // max |V| for the stability bound
+    rc = ensure_partial(c, 1024);
+    if (rc) return rc;
+    if (c->dtype == TDSE_F32)
+        absmax_partial_kernel<float><<<256, 256, 0, c->stream>>>(static_cast<const float*>((void*)entry_ptr(c, c->V, b0)), c->g.cells, c->partial);
+    else
+        absmax_partial_kernel<double><<<256, 256, 0, c->stream>>>(static_cast<const double*>((void*)entry_ptr(c, c->V, b0)), c->g.cells, c->partial);
+    CU_LAUNCH_CHECK(c);
+    double part[256];
+    CU_TRY(c, cudaMemcpyAsync(part, c->partial, sizeof(part), cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    for (double v : part) c->vabs_max = std::max(c->vabs_max, v);
+    return TDSE_OK;
+}
+
+int tdse_set_wavepacket(tdse_ctx* c, int b, double x0, double y0, double z0, double sigma,
+                        double kx, double ky, double kz, double amplitude)
+{
+    if (!c) return TDSE_EINVAL;
+    if (!(sigma > 0)) return fail(c, TDSE_EINVAL, "tdse_set_wavepacket: sigma must be > 0");
+    int b0, b1;
+    if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_wavepacket: entry out of range");
+    if (!c->ws) return fail(c, TDSE_ESTATE, "tdse_set_wavepacket: set the potential first (the staggered start needs V)");
+    for (int e = b0; e < b1; ++e)
+        if (!c->have_V[e]) return fail(c, TDSE_ESTATE, "tdse_set_wavepacket: set the potential first (the staggered start needs V)");
+    const double pi = 3.14159265358979323846;
+    PacketParams p;
+    p.x0 = x0; p.y0 = y0; p.z0 = z0; p.inv2s2 = 1.0 / (2.0 * sigma * sigma);
+    p.kx = kx; p.ky = ky; p.kz = kz;
+    p.amp = amplitude != 0.0 ? amplitude : std::pow(pi * sigma * sigma, -0.75);
+    const unsigned nblk = (unsigned)((c->g.cells + 255) / 256);
+    for (int e = b0; e < b1; ++e) {
+        if (c->dtype == TDSE_F32)
+            wavepacket_init_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->dx, p, c->c, c->cv,
+                (const float*)entry_ptr(c, c->V, e), (float*)entry_ptr(c, c->R[c->cur], e), (float*)entry_ptr(c, c->I[c->cur], e));
+        else
+            wavepacket_init_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->dx, p, c->c, c->cv,
+                (const double*)entry_ptr(c, c->V, e), (double*)entry_ptr(c, c->R[c->cur], e), (double*)entry_ptr(c, c->I[c->cur], e));
+        CU_LAUNCH_CHECK(c);
+        c->have_state[e] = 1;
+    }
+    return reset_detector(c);
+}
+
+int tdse_set_state(tdse_ctx* c, int b, const void* R, const void* I_half, int on_device)
+{
+    if (!c) return TDSE_EINVAL;
+    if (!R || !I_half) return fail(c, TDSE_EINVAL, "tdse_set_state: NULL state");
+    int b0, b1;
+    if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_state: entry out of range");
+    int rc = ensure_workspace(c);
+    if (rc) return rc;
+    const size_t nbytes = (size_t)c->g.cells * c->w;
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    for (int e = b0; e < b1; ++e) {
+        CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->R[c->cur], e), R, nbytes, kind, c->stream));
+        CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->I[c->cur], e), I_half, nbytes, kind, c->stream));
+        c->have_state[e] = 1;
+    }
+    if (!on_device) CU_TRY(c, cudaStreamSynchronize(c->stream));   // caller may reuse pageable buffers
+    return reset_detector(c);
+}
+
+int tdse_set_detector(tdse_ctx* c, int k_plane, int every, int max_samples)
+{
+    if (!c) return TDSE_EINVAL;
+    if (every < 0 || max_samples < 0) return fail(c, TDSE_EINVAL, "tdse_set_detector: every, max_samples must be >= 0");
+    if (every > 0 && (k_plane < 0 || k_plane >= c->g.nz)) return fail(c, TDSE_EINVAL, "tdse_set_detector: plane out of range");
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    if (c->trace) { cudaFree(c->trace); c->trace = nullptr; }
+    c->k_det = k_plane; c->every = every; c->max_samples = max_samples;
+    if (max_samples > 0) CU_TRY(c, cudaMalloc(&c->trace, (size_t)c->g.batch * max_samples * sizeof(double)));
+    return reset_detector(c);
+}
+
+int tdse_step(tdse_ctx* c, int n)
+{
+    if (!c) return TDSE_EINVAL;
+    if (n < 0) return fail(c, TDSE_EINVAL, "tdse_step: n < 0");
+    if (!c->ws) return fail(c, TDSE_ESTATE, "tdse_step: potential and state are not set");
+    for (int e = 0; e < c->g.batch; ++e)
+        if (!c->have_V[e] || !c->have_state[e]) return fail(c, TDSE_ESTATE, "tdse_step: potential and state must be set for every entry");
+    if (!c->allow_unstable) {
+        const double bound = 2.0 * c->hbar / (12.0 * c->hbar * c->hbar / (2.0 * c->mass * c->dx * c->dx) + c->vabs_max);
+        if (c->dt > bound) {
+            char buf[200];
+            std::snprintf(buf, sizeof buf, "tdse_step: dt = %.6g exceeds the stability bound %.6g (max|V| = %.6g)", c->dt, bound, c->vabs_max);
+            return fail(c, TDSE_EUNSTABLE, buf);
+        }
+    }
+    int kernel = c->opt_kernel;
+    if (kernel == TDSE_KERNEL_AUTO) kernel = fused_supported(c) ? TDSE_KERNEL_FUSED : TDSE_KERNEL_TWOPASS;
+    if (kernel == TDSE_KERNEL_FUSED && !fused_supported(c))
+        return fail(c, TDSE_EINVAL, "tdse_step: fused kernel needs a 5-array workspace and nx divisible by 16 bytes / element size");
+    const int tmax = (c->opt_tblock > 0) ? c->opt_tblock : 2;
+    c->last_kernel = kernel;
+    int remaining = n;
+    while (remaining > 0) {
+        const int to_sample = (c->every > 0) ? (int)(c->every - (c->steps % c->every)) : std::numeric_limits<int>::max();
+        int rc;
+        if (kernel == TDSE_KERNEL_TWOPASS) {
+            rc = (c->dtype == TDSE_F32) ? launch_twopass_step<float>(c) : launch_twopass_step<double>(c);
+            if (rc) return rc;
+            c->steps += 1; remaining -= 1;
+            c->last_tblock = 1;
+            if (to_sample == 1) {
+                rc = (c->dtype == TDSE_F32) ? sample_detector_twopass<float>(c) : sample_detector_twopass<double>(c);
+                if (rc) return rc;
+            }
+        } else {
+            const int T = std::min(std::min(tmax, remaining), to_sample);
+            const bool sample = (T == to_sample);
+            FusedParams P{};
+            P.Rin = c->R[c->cur]; P.Iin = c->I[c->cur]; P.V = c->V;
+            P.Rout = c->R[c->cur ^ 1]; P.Iout = c->I[c->cur ^ 1];
+            P.mask = c->mask_dev;
+            P.nx = c->g.nx; P.ny = c->g.ny; P.nz = c->g.nz; P.batch = c->g.batch;
+            P.bcx = c->g.bcx; P.bcy = c->g.bcy; P.bcz = c->g.bcz;
+            P.c = c->c; P.cv = c->cv;
+            P.sample = sample ? 1 : 0; P.k_det = c->k_det; P.D = c->D;
+            if (sample) {
+                const size_t max_tiles = (size_t)((c->g.nx + 15) / 16) * ((c->g.ny + 7) / 8);   // tiles are never smaller than 16 x 8
+                rc = ensure_partial(c, (size_t)c->g.batch * max_tiles);
+                if (rc) return rc;
+            }
+            P.partial = c->partial;
+            rc = launch_fused(c, P, T);
+            if (rc) return rc;
+            c->cur ^= 1;
+            c->steps += T; remaining -= T;
+            c->last_tblock = T;
+            if (sample) {
+                rc = finish_trace(c, P.tiles_x * P.tiles_y);
+                if (rc) return rc;
+            }
+        }
+    }
+    return TDSE_OK;
+}
+
+int tdse_detector_read(tdse_ctx* c, int b, double* image_host, double* trace_host, int cap, int* nsamples)
+{
+    if (!c) return TDSE_EINVAL;
+    if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_detector_read: entry out of range");
+    if (cap < 0) return fail(c, TDSE_EINVAL, "tdse_detector_read: cap < 0");
+    if (image_host)
+        CU_TRY(c, cudaMemcpyAsync(image_host, c->D + (size_t)b * c->g.plane, (size_t)c->g.plane * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    const int ntr = std::min(std::min(cap, c->nsamples), c->max_samples);
+    if (trace_host && ntr > 0)
+        CU_TRY(c, cudaMemcpyAsync(trace_host, c->trace + (size_t)b * c->max_samples, (size_t)ntr * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    if (nsamples) *nsamples = c->nsamples;
+    return TDSE_OK;
+}
+
+int tdse_detector_device(tdse_ctx* c, double** image_device, double** trace_device, int* max_samples)
+{
+    if (!c) return TDSE_EINVAL;
+    if (image_device) *image_device = c->D;
+    if (trace_device) *trace_device = c->trace;
+    if (max_samples) *max_samples = c->max_samples;
+    return TDSE_OK;
+}
+
+int tdse_read_psi(tdse_ctx* c, int b, void* R_host, void* I_host)
+{
+    if (!c) return TDSE_EINVAL;
+    if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_read_psi: entry out of range");
+    if (!c->ws || !c->have_state[b]) return fail(c, TDSE_ESTATE, "tdse_read_psi: state not set");
+    const size_t nbytes = (size_t)c->g.cells * c->w;
+    if (R_host) CU_TRY(c, cudaMemcpyAsync(R_host, entry_ptr(c, c->R[c->cur], b), nbytes, cudaMemcpyDeviceToHost, c->stream));
+    if (I_host) CU_TRY(c, cudaMemcpyAsync(I_host, entry_ptr(c, c->I[c->cur], b), nbytes, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    return TDSE_OK;
+}
+
+int tdse_read_potential(tdse_ctx* c, int b, void* V_host)
+{
+    if (!c) return TDSE_EINVAL;
+    if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_read_potential: entry out of range");
+    if (!c->ws || !c->have_V[b]) return fail(c, TDSE_ESTATE, "tdse_read_potential: potential not set");
+    if (!V_host) return fail(c, TDSE_EINVAL, "tdse_read_potential: NULL");
+    CU_TRY(c, cudaMemcpyAsync(V_host, entry_ptr(c, c->V, b), (size_t)c->g.cells * c->w, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    return TDSE_OK;
+}
+
+int tdse_norm(tdse_ctx* c, int b, double* q_visscher, double* q_paper)
+{
+    if (!c) return TDSE_EINVAL;
+    if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_norm: entry out of range");
+    if (!c->ws || !c->have_state[b] || !c->have_V[b]) return fail(c, TDSE_ESTATE, "tdse_norm: potential and state must be set");
+    const unsigned nblk = (unsigned)((c->g.cells + 255) / 256);
+    int rc = ensure_partial(c, (size_t)2 * nblk);
+    if (rc) return rc;
+    if (c->dtype == TDSE_F32)
+        norm_partial_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->c, c->cv, (const float*)entry_ptr(c, c->V, b),
+            (const float*)c->mask_dev, (const float*)entry_ptr(c, c->R[c->cur], b), (const float*)entry_ptr(c, c->I[c->cur], b), c->partial);
+    else
+        norm_partial_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->c, c->cv, (const double*)entry_ptr(c, c->V, b),
+            (const double*)c->mask_dev, (const double*)entry_ptr(c, c->R[c->cur], b), (const double*)entry_ptr(c, c->I[c->cur], b), c->partial);
+    CU_LAUNCH_CHECK(c);
+    reduce_rows_kernel<<<1, 256, 0, c->stream>>>(c->partial, (int)nblk, 2, c->dx * c->dx * c->dx, c->scalars);
+    CU_LAUNCH_CHECK(c);
+    double q[2];
+    CU_TRY(c, cudaMemcpyAsync(q, c->scalars, sizeof q, cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    if (q_visscher) *q_visscher = q[0];
+    if (q_paper) *q_paper = q[1];
+    return TDSE_OK;
+}
+
+int tdse_set_option(tdse_ctx* c, const char* key, long long value)
+{
+    if (!c || !key) return TDSE_EINVAL;
+    const std::string k(key);
+    if (k == "kernel") {
+        if (value < TDSE_KERNEL_AUTO || value > TDSE_KERNEL_FUSED) return fail(c, TDSE_EINVAL, "tdse_set_option: kernel");
+        c->opt_kernel = (int)value;
+    } else if (k == "tblock") {
+        if (value < 0 || value > 2) return fail(c, TDSE_EINVAL, "tdse_set_option: tblock must be 0..2");
+        c->opt_tblock = (int)value;
+    } else if (k == "allow_unstable") {
+        c->allow_unstable = value ? 1 : 0;
+    } else {
+        return fail(c, TDSE_EINVAL, "tdse_set_option: unknown key " + k);
+    }
+    return TDSE_OK;
+}
+
+int tdse_get_info(const tdse_ctx* c, const char* key, long long* value)
+{
+    if (!c || !key || !value) return TDSE_EINVAL;
+    const std::string k(key);
+    if (k == "launches") *value = c->launches;
+    else if (k == "steps") *value = c->steps;
+    else if (k == "kernel") *value = c->last_kernel;
+    else if (k == "tblock") *value = c->last_tblock;
+    else if (k == "pingpong") *value = c->pingpong ? 1 : 0;
+    else if (k == "tile_x") *value = c->last_tile_x;
+    else if (k == "tile_y") *value = c->last_tile_y;
+    else if (k == "z_chunks") *value = c->last_chunks;
+    else if (k == "nsamples") *value = c->nsamples;
+    else return TDSE_EINVAL;
+    return TDSE_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,262 @@
+// tdse_kernels_basic.cuh -- set-up kernels (potential, packet, raw fills), the two-pass
+// reference stencil (one thread per cell), detector and norm reductions.
+// Citations: PAPER.md = /root/reference/PAPER.md (arXiv 2401.07416).
+#pragma once
+#include "tdse_common.cuh"
+
+namespace tdse {
+
+struct AtomRec { double x, y, z, Z, soft2, screen; };   // same layout as tdse_atom
+
+// ---------------------------------------------------------------------------------------------
+// S0 potential build (BASELINE.json north_star (1)): V = clamp(sum_a -Z_a exp(-r_a/lambda_a)/sqrt(r_a^2+s_a^2)).
+// One thread per cell, x fastest; atoms staged through shared memory in chunks; double accumulate in
+// list order; one rounding to `real`.  Nearest image on periodic axes.
+// ---------------------------------------------------------------------------------------------
+constexpr int kAtomChunk = 128;
+
+template <typename real>
+__global__ void __launch_bounds__(256)
+potential_build_kernel(Grid g, double dx, const AtomRec* __restrict__ atoms, int natoms,
+                       double vmin, double vmax, double rcut, real* __restrict__ V /* entry base */)
+{
+    __shared__ AtomRec s_atoms[kAtomChunk];
+    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = cell < g.cells;
+    int i = 0, j = 0, k = 0;
+    if (live) {
+        i = (int)(cell % g.nx);
+        const long long t = cell / g.nx;
+        j = (int)(t % g.ny);
+        k = (int)(t / g.ny);
+    }
+    const double x = i * dx, y = j * dx, z = k * dx;
+    const double Lx = g.nx * dx, Ly = g.ny * dx, Lz = g.nz * dx;
+    double sum = 0.0;
+    for (int a0 = 0; a0 < natoms; a0 += kAtomChunk) {
+        const int na = min(kAtomChunk, natoms - a0);
+        __syncthreads();
+        for (int q = threadIdx.x; q < na * 6; q += blockDim.x)
+            reinterpret_cast<double*>(s_atoms)[q] = reinterpret_cast<const double*>(atoms + a0)[q];
+        __syncthreads();
+        if (live) {
+            for (int a = 0; a < na; ++a) {
+                const AtomRec A = s_atoms[a];
+                double ddx = x - A.x, ddy = y - A.y, ddz = z - A.z;
+                if (g.bcx == BC_PERIODIC) ddx = ddx - Lx * round(ddx / Lx);
+                if (g.bcy == BC_PERIODIC) ddy = ddy - Ly * round(ddy / Ly);
+                if (g.bcz == BC_PERIODIC) ddz = ddz - Lz * round(ddz / Lz);
+                const double r2 = ddx * ddx + ddy * ddy + ddz * ddz;
+                const double r = sqrt(r2);
+                if (rcut > 0.0 && r > rcut) continue;
+                double screen = 1.0;
+                if (A.screen > 0.0 && isfinite(A.screen)) screen = exp(-r / A.screen);
+                sum += -A.Z * screen / sqrt(r2 + A.soft2);
+            }
+        }
+    }
+    if (live) {
+        sum = fmin(fmax(sum, vmin), vmax);
+        V[cell] = (real)sum;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// S1 packet init: eq (3) PAPER.md:52 with signed wave vector; staggered start
+//   R^0 = Re psi0,  I^{-1/2} = Im psi0 + (1/2) A Re psi0,  A f = -c d2 f + c_v V f   (reading 4)
+// evaluated in double from the stored V; neighbours of Re psi0 are re-evaluated analytically at the
+// (wrapped) neighbour grid point, or are 0 beyond a Dirichlet face.
+// ---------------------------------------------------------------------------------------------
+struct PacketParams { double x0, y0, z0, inv2s2, kx, ky, kz, amp; };
+
+__device__ __forceinline__ void packet_eval(const PacketParams& p, double dx, int i, int j, int k,
+                                            double* re, double* im)
+{
+    const double ddx = i * dx - p.x0, ddy = j * dx - p.y0, ddz = k * dx - p.z0;
+    const double G = p.amp * exp(-(ddx * ddx + ddy * ddy + ddz * ddz) * p.inv2s2);
+    const double phi = p.kx * ddx + p.ky * ddy + p.kz * ddz;
+    double s, c;
+    sincos(phi, &s, &c);
+    *re = G * c;
+    *im = G * s;
+}
+
+__device__ __forceinline__ double packet_re_nbr(const PacketParams& p, const Grid& g, double dx,
+                                                int i, int j, int k)
+{
+    if (i < 0 || i >= g.nx) { if (g.bcx == BC_PERIODIC) i = wrap_index(i, g.nx); else return 0.0; }
+    if (j < 0 || j >= g.ny) { if (g.bcy == BC_PERIODIC) j = wrap_index(j, g.ny); else return 0.0; }
+    if (k < 0 || k >= g.nz) { if (g.bcz == BC_PERIODIC) k = wrap_index(k, g.nz); else return 0.0; }
+    double re, im;
+    packet_eval(p, dx, i, j, k, &re, &im);
+    return re;
+}
+
+template <typename real>
+__global__ void __launch_bounds__(256)
+wavepacket_init_kernel(Grid g, double dx, PacketParams p, double c, double cv,
+                       const real* __restrict__ V, real* __restrict__ R, real* __restrict__ I)
+{
+    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= g.cells) return;
+    const int i = (int)(cell % g.nx);
+    const long long t = cell / g.nx;
+    const int j = (int)(t % g.ny);
+    const int k = (int)(t / g.ny);
+    double re, im;
+    packet_eval(p, dx, i, j, k, &re, &im);
+    const double d2x = packet_re_nbr(p, g, dx, i + 1, j, k) - 2.0 * re + packet_re_nbr(p, g, dx, i - 1, j, k);
+    const double d2y = packet_re_nbr(p, g, dx, i, j + 1, k) - 2.0 * re + packet_re_nbr(p, g, dx, i, j - 1, k);
+    const double d2z = packet_re_nbr(p, g, dx, i, j, k + 1) - 2.0 * re + packet_re_nbr(p, g, dx, i, j, k - 1);
+    const double Ar = -c * d2x - c * d2y - c * d2z + cv * (double)V[cell] * re;
+    R[cell] = (real)re;
+    I[cell] = (real)(im + 0.5 * Ar);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Two-pass reference stencil: one thread per cell, neighbours straight from global memory (L1/L2).
+//   sgn = +1: eq (9) PAPER.md:83  dst = I, src = R;   sgn = -1: eq (8) PAPER.md:74  dst = R, src = I
+//   dst <- M[k] * ( dst + sgn * ( c * (sum of 6 neighbours - 6 src) - c_v V src ) )
+// In place is safe (dst is read only at the thread's own cell).  Works for every shape and boundary
+// combination; the fused kernels in tdse_kernels_fused.cuh are the fast path.
+// ---------------------------------------------------------------------------------------------
+template <typename real>
+__device__ __forceinline__ real load_nbr(const real* __restrict__ f, const Grid& g, int i, int j, int k)
+{
+    if (i < 0)     { if (g.bcx == BC_PERIODIC) i = g.nx - 1; else return (real)0; }
+    if (i >= g.nx) { if (g.bcx == BC_PERIODIC) i = 0;        else return (real)0; }
+    if (j < 0)     { if (g.bcy == BC_PERIODIC) j = g.ny - 1; else return (real)0; }
+    if (j >= g.ny) { if (g.bcy == BC_PERIODIC) j = 0;        else return (real)0; }
+    if (k < 0)     { if (g.bcz == BC_PERIODIC) k = g.nz - 1; else return (real)0; }
+    if (k >= g.nz) { if (g.bcz == BC_PERIODIC) k = 0;        else return (real)0; }
+    return f[((long long)k * g.ny + j) * g.nx + i];
+}
+
+template <typename real>
+__global__ void __launch_bounds__(256)
+half_step_kernel(Grid g, real c, real cv, real sgn, const real* __restrict__ V,
+                 const real* __restrict__ M, const real* __restrict__ src, real* __restrict__ dst)
+{
+    // grid: x = cells of one entry / 256, y = batch entry
+    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= g.cells) return;
+    const long long base = (long long)blockIdx.y * g.cells;
+    const int i = (int)(cell % g.nx);
+    const long long t = cell / g.nx;
+    const int j = (int)(t % g.ny);
+    const int k = (int)(t / g.ny);
+    const real* s = src + base;
+    const real s0 = s[cell];
+    const real nb = (load_nbr(s, g, i + 1, j, k) + load_nbr(s, g, i - 1, j, k))
+                  + (load_nbr(s, g, i, j + 1, k) + load_nbr(s, g, i, j - 1, k))
+                  + (load_nbr(s, g, i, j, k + 1) + load_nbr(s, g, i, j, k - 1));
+    const real lap = nb - (real)6 * s0;
+    const real upd = c * lap - cv * V[base + cell] * s0;
+    dst[base + cell] = M[k] * (dst[base + cell] + sgn * upd);
+}
+
+// ---------------------------------------------------------------------------------------------
+// S5 detector (eq (15), density of PAPER.md:87): D += R^2 + I^2 on plane k_det,
+// per-block partial sums (double) -> trace_finish_kernel sums them in fixed order.
+// grid: x = ceil(nx*ny / 256), y = batch.
+// ---------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void __launch_bounds__(256)
+detector_accum_kernel(Grid g, int k_det, const real* __restrict__ R, const real* __restrict__ I,
+                      double* __restrict__ D, double* __restrict__ partial /* [batch][gridDim.x] */)
+{
+    __shared__ double scratch[32];
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    double rho = 0.0;
+    if (p < g.plane) {
+        const long long off = (long long)blockIdx.y * g.cells + (long long)k_det * g.plane + p;
+        const double r = (double)R[off], im = (double)I[off];
+        rho = r * r + im * im;
+        D[(long long)blockIdx.y * g.plane + p] += rho;
+    }
+    const double s = block_sum(rho, scratch);
+    if (threadIdx.x == 0) partial[(long long)blockIdx.y * gridDim.x + blockIdx.x] = s;
+}
+
+// trace[b][slot] = scale * sum_{q < nparts} partial[b][q]  (serial, fixed order).  One thread per entry.
+__global__ void trace_finish_kernel(const double* __restrict__ partial, int nparts, double scale,
+                                    double* __restrict__ trace, int max_samples, int slot, int batch)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    double s = 0.0;
+    for (int q = 0; q < nparts; ++q) s += partial[(long long)b * nparts + q];
+    if (slot < max_samples) trace[(long long)b * max_samples + slot] = scale * s;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Diagnostics: q_paper = sum R^2 + I^2, q_visscher = sum R^2 + I(+) I with a look-ahead eq (9) in double.
+// One entry at a time; per-block partials [2][gridDim.x]; reduce_pairs_kernel finishes.
+// ---------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void __launch_bounds__(256)
+norm_partial_kernel(Grid g, double c, double cv, const real* __restrict__ V, const real* __restrict__ M,
+                    const real* __restrict__ R, const real* __restrict__ I, double* __restrict__ partial)
+{
+    __shared__ double scratch[32];
+    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    double qv = 0.0, qp = 0.0;
+    if (cell < g.cells) {
+        const int i = (int)(cell % g.nx);
+        const long long t = cell / g.nx;
+        const int j = (int)(t % g.ny);
+        const int k = (int)(t / g.ny);
+        const double r0 = (double)R[cell], i0 = (double)I[cell];
+        const double nb = ((double)load_nbr(R, g, i + 1, j, k) + (double)load_nbr(R, g, i - 1, j, k))
+                        + ((double)load_nbr(R, g, i, j + 1, k) + (double)load_nbr(R, g, i, j - 1, k))
+                        + ((double)load_nbr(R, g, i, j, k + 1) + (double)load_nbr(R, g, i, j, k - 1));
+        const double ip = (double)M[k] * (i0 + c * (nb - 6.0 * r0) - cv * (double)V[cell] * r0);
+        qv = r0 * r0 + ip * i0;
+        qp = r0 * r0 + i0 * i0;
+    }
+    const double sv = block_sum(qv, scratch);
+    const double sp = block_sum(qp, scratch);
+    if (threadIdx.x == 0) {
+        partial[blockIdx.x] = sv;
+        partial[gridDim.x + blockIdx.x] = sp;
+    }
+}
+
+// out[r] = scale * sum_q partial[r*n + q], r = 0..rows-1; single block, fixed order per thread stripe.
+__global__ void __launch_bounds__(256)
+reduce_rows_kernel(const double* __restrict__ partial, int n, int rows, double scale, double* __restrict__ out)
+{
+    __shared__ double scratch[32];
+    for (int r = 0; r < rows; ++r) {
+        double s = 0.0;
+        for (int q = threadIdx.x; q < n; q += blockDim.x) s += partial[(long long)r * n + q];
+        s = block_sum(s, scratch);
+        if (threadIdx.x == 0) out[r] = scale * s;
+    }
+}
+
+// max |V| over one entry (for the stability bound after a raw-grid upload).
+template <typename real>
+__global__ void __launch_bounds__(256)
+absmax_partial_kernel(const real* __restrict__ V, long long n, double* __restrict__ partial)
+{
+    __shared__ double s_max[256];
+    double m = 0.0;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (long long)gridDim.x * blockDim.x)
+        m = fmax(m, fabs((double)V[q]));
+    s_max[threadIdx.x] = m;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) s_max[threadIdx.x] = fmax(s_max[threadIdx.x], s_max[threadIdx.x + o]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = s_max[0];
+}
+
+__global__ void fill_zero_kernel(double* p, long long n)
+{
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (long long)gridDim.x * blockDim.x)
+        p[q] = 0.0;
+}
+
+}  // namespace tdse

@@ -1,0 +1,321 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances (BASELINE.json north_star): relative L2 error on psi and on the
+detector image <= 1e-11 for fp64 contexts and <= 1e-4 for fp32 contexts.  For fp32 the truth is the
+oracle run in double on the same float-rounded inputs (V, mask, psi0, coefficients).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import OracleRun
+from workloads import make_config, random_state, random_potential, PERIODIC, DIRICHLET
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-11, "f32": 1e-4}
+TWOPASS, FUSED = 1, 2
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64).ravel()
+    b = np.asarray(b, dtype=np.float64).ravel()
+    nb = np.linalg.norm(b)
+    return float(np.linalg.norm(a - b) / nb) if nb > 0 else float(np.linalg.norm(a))
+
+
+def make_ctx(nx, ny, nz, batch, dx, dt, dtype, **kw):
+    from paper_2401_07416_b200 import Tdse
+    return Tdse(nx, ny, nz, batch, dx, dt, 1.0, 1.0, dtype, **kw)
+
+
+def oracle_for(w, entry, steps):
+    return OracleRun.from_workload(w, entry=entry, dtype="f64",
+                                   round_to="f32" if w.dtype == "f32" else None).step(steps)
+
+
+# ------------------------------------------------------------------------------------------
+# S0 / S1: potential builder and packet init
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("idx,shape", [(0, (24, 20, 28)), (1, (40, 36, 48)), (3, (36, 40, 44)), (4, (48, 40, 56))])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_potential_and_packet_match_oracle(idx, shape, dtype):
+    from paper_2401_07416_b200 import Tdse
+    w = make_config(idx, n=shape, batch=2 if idx == 3 else 1, dtype=dtype)
+    t = Tdse.from_workload(w)
+    for b in range(w.batch):
+        o = OracleRun.from_workload(w, entry=b, dtype="f64", round_to="f32" if dtype == "f32" else None)
+        V = t.read_potential(b)
+        R, I = t.read_psi(b)
+        if dtype == "f64":
+            assert np.max(np.abs(V - o.V64)) <= 1e-13 * max(1.0, np.max(np.abs(o.V64)))
+            assert rel_l2(R, o.R) < 1e-14 and rel_l2(I, o.I) < 1e-14
+        else:
+            # one rounding of a double result that may differ in its last bits: at most 1 ulp
+            ulp = np.spacing(np.abs(o.V).astype(np.float32)).astype(np.float64)
+            assert np.all(np.abs(V.astype(np.float64) - o.V) <= ulp)
+            assert rel_l2(R, o.R) < 1e-7 and rel_l2(I, o.I) < 1e-7
+        assert V.min() >= w.vmin and V.max() <= w.vmax
+    t.close()
+
+
+# ------------------------------------------------------------------------------------------
+# S2-S5: the recurrence on raw seeded states, every boundary combination, awkward sizes
+# ------------------------------------------------------------------------------------------
+BCS = [(PERIODIC, PERIODIC, DIRICHLET), (DIRICHLET, DIRICHLET, DIRICHLET), (PERIODIC, PERIODIC, PERIODIC),
+       (DIRICHLET, PERIODIC, PERIODIC), (PERIODIC, DIRICHLET, DIRICHLET)]
+SHAPES = [(72, 40, 37), (64, 64, 16), (8, 6, 5), (136, 70, 21), (4, 3, 2)]
+VARIANTS = [(TWOPASS, 1), (FUSED, 1), (FUSED, 2)]
+
+
+@pytest.mark.parametrize("kernel,tblock", VARIANTS)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape,bc", list(zip(SHAPES, BCS)) + [((40, 24, 30), BCS[2]), ((40, 24, 30), BCS[1])])
+def test_recurrence_matches_oracle_on_random_states(kernel, tblock, dtype, shape, bc):
+    nx, ny, nz = shape
+    dx, dt, steps, batch = 0.25, 0.004, 23, 2
+    absorb = min(4, nz // 3)
+    t = make_ctx(nx, ny, nz, batch, dx, dt, dtype)
+    t.set_boundary(*bc, absorb, absorb, 0.07, 2)
+    t.set_option("kernel", kernel)
+    t.set_option("tblock", tblock)
+    k_det = min(3, nz - 1)
+    t.set_detector(k_det, 5, 8)
+    ora = []
+    for b in range(batch):
+        V = random_potential(100 + b, (nz, ny, nx), -30.0, 5.0)
+        R0, I0 = random_state(200 + b, (nz, ny, nx))
+        t.set_potential_grid(b, V.astype(t.np_dtype))
+        t.set_state(b, R0.astype(t.np_dtype), I0.astype(t.np_dtype))
+        o = OracleRun(nx, ny, nz, dx, dt, bc=bc, absorb_lo=absorb, absorb_hi=absorb, strength=0.07,
+                      round_to="f32" if dtype == "f32" else None)
+        o.set_potential_grid(V).set_state(R0, I0).set_detector(k_det, 5)
+        ora.append(o.step(steps))
+    t.step(steps)
+    assert t.get_info("kernel") == kernel and t.get_info("steps") == steps
+    for b in range(batch):
+        R, I = t.read_psi(b)
+        D, tr = t.detector_read(b)
+        tol = TOL[dtype]
+        assert rel_l2(R, ora[b].R) < tol and rel_l2(I, ora[b].I) < tol
+        assert len(tr) == 4 and rel_l2(D, ora[b].D) < tol and rel_l2(tr, ora[b].trace) < tol
+    t.close()
+
+
+@pytest.mark.parametrize("kernel,tblock", VARIANTS)
+def test_step_counts_split_across_calls_and_odd_sampling_period(kernel, tblock):
+    """n steps in one call == the same steps in uneven pieces; `every` odd forces T=1 launches in between."""
+    w = make_config(1, n=(40, 32, 48), steps=0)
+    from paper_2401_07416_b200 import Tdse
+    a, b = Tdse.from_workload(w), Tdse.from_workload(w)
+    for t in (a, b):
+        t.set_option("kernel", kernel); t.set_option("tblock", tblock)
+        t.set_detector(7, 3, 32)
+    a.step(31)
+    for n in (1, 2, 5, 0, 7, 16):
+        b.step(n)
+    Ra, Ia = a.read_psi(0); Rb, Ib = b.read_psi(0)
+    Da, ta = a.detector_read(0); Db, tb = b.detector_read(0)
+    assert len(ta) == len(tb) == 10
+    assert np.array_equal(Da, Db) and np.array_equal(ta, tb)
+    if kernel == TWOPASS or tblock == 1:
+        assert np.array_equal(Ra, Rb) and np.array_equal(Ia, Ib)     # same arithmetic, same order
+    else:
+        assert rel_l2(Ra, Rb) < 1e-13 and rel_l2(Ia, Ib) < 1e-13     # T=2 vs T=1 launches regroup nothing either
+    o = OracleRun.from_workload(w)
+    o.set_detector(7, 3).step(31)
+    assert rel_l2(Ra, o.R) < 1e-11 and rel_l2(Da, o.D) < 1e-11 and rel_l2(ta, o.trace) < 1e-11
+    a.close(); b.close()
+
+
+def test_identical_entries_give_bitwise_identical_results_at_any_batch_position():
+    w = make_config(3, n=(64, 48, 40), batch=1, steps=0)
+    from paper_2401_07416_b200 import Tdse
+    w5 = w.with_(batch=5, atoms=[w.atoms[0]] * 5)
+    t = Tdse.from_workload(w5)
+    t.step(24)
+    R0, I0 = t.read_psi(0)
+    D0, tr0 = t.detector_read(0)
+    for b in (1, 4):
+        R, I = t.read_psi(b)
+        D, tr = t.detector_read(b)
+        assert np.array_equal(R, R0) and np.array_equal(I, I0) and np.array_equal(D, D0) and np.array_equal(tr, tr0)
+    t.close()
+
+
+def test_fused_and_twopass_agree_and_conserve_the_visscher_norm():
+    w = make_config(0, n=(48, 40, 56), steps=0)
+    from paper_2401_07416_b200 import Tdse
+    out = {}
+    for kernel in (TWOPASS, FUSED):
+        t = Tdse.from_workload(w)
+        t.set_option("kernel", kernel)
+        q0 = t.norm(0)
+        t.step(200)
+        q1 = t.norm(0)
+        assert abs(q1[0] - q0[0]) / q0[0] < 1e-12          # conserved exactly by the scheme (no mask in cfg 0)
+        out[kernel] = t.read_psi(0)
+        t.close()
+    assert rel_l2(out[FUSED][0], out[TWOPASS][0]) < 1e-12
+    o = OracleRun.from_workload(w)
+    assert abs(o.norm()[0] - q0[0]) / q0[0] < 1e-13
+
+
+# ------------------------------------------------------------------------------------------
+# the BASELINE configurations (reduced grid / full steps where the oracle finishes in seconds)
+# ------------------------------------------------------------------------------------------
+def _run_config(w, steps, entries=None):
+    from paper_2401_07416_b200 import Tdse
+    t = Tdse.from_workload(w)
+    t.step(steps)
+    worst = 0.0
+    for b in (entries if entries is not None else range(w.batch)):
+        R, I = t.read_psi(b)
+        D, tr = t.detector_read(b)
+        o = oracle_for(w, b, steps)
+        errs = (rel_l2(R, o.R), rel_l2(I, o.I), rel_l2(D, o.D), rel_l2(tr, o.trace))
+        worst = max(worst, *errs)
+        assert len(tr) == len(o.trace) == steps // w.every
+    info = (t.get_info("kernel"), t.get_info("tblock"))
+    t.close()
+    return worst, info
+
+
+def test_config0_full_size_full_steps():
+    w = make_config(0)
+    worst, info = _run_config(w, w.steps)
+    assert info == (FUSED, 2)
+    assert worst < 1e-11
+
+
+def test_config1_full_size_full_steps():
+    w = make_config(1)
+    worst, info = _run_config(w, w.steps)
+    assert info == (FUSED, 2)
+    assert worst < 1e-11
+
+
+def test_config2_reduced_grid():
+    w = make_config(2, n=(64, 64, 128), steps=800)
+    worst, _ = _run_config(w, w.steps)
+    assert worst < 1e-4
+
+
+def test_config3_reduced_batch_and_grid():
+    w = make_config(3, n=(64, 64, 64), batch=6, steps=600)
+    worst, _ = _run_config(w, w.steps, entries=(0, 3, 5))
+    assert worst < 1e-4
+
+
+def test_config4_reduced_grid_fp32_vs_fp64_detector_agreement():
+    from paper_2401_07416_b200 import Tdse
+    imgs = {}
+    for dtype in ("f32", "f64"):
+        w = make_config(4, n=(64, 64, 96), dtype=dtype, steps=400, batch=2)
+        worst, _ = _run_config(w, w.steps)
+        assert worst < TOL[dtype]
+        t = Tdse.from_workload(w)
+        t.step(w.steps)
+        imgs[dtype] = t.detector_read(1)[0]
+        t.close()
+    assert rel_l2(imgs["f32"], imgs["f64"]) < 1e-4
+
+
+# ------------------------------------------------------------------------------------------
+# edge cases and error behaviour of the boundary
+# ------------------------------------------------------------------------------------------
+def test_call_order_and_stability_errors():
+    from paper_2401_07416_b200 import Tdse, TdseError, TDSE_ESTATE, TDSE_EUNSTABLE, TDSE_EINVAL
+    t = make_ctx(16, 16, 16, 1, 0.2, 0.004, "f64")
+    with pytest.raises(TdseError) as e:
+        t.step(1)
+    assert e.value.code == TDSE_ESTATE
+    with pytest.raises(TdseError) as e:
+        t.set_wavepacket(0, 1.6, 1.6, 1.6, 0.5, 0, 0, 1.0)
+    assert e.value.code == TDSE_ESTATE
+    t.set_potential(0, np.zeros((0, 6)), -1.0, 0.0)
+    with pytest.raises(TdseError) as e:
+        t.step(1)
+    assert e.value.code == TDSE_ESTATE
+    t.set_wavepacket(0, 1.6, 1.6, 1.6, 0.5, 0, 0, 1.0)
+    t.step(0)
+    t.step(3)
+    with pytest.raises(TdseError) as e:
+        t.set_potential(3, np.zeros((0, 6)), -1.0, 0.0)
+    assert e.value.code == TDSE_EINVAL
+    with pytest.raises(TdseError) as e:
+        t.set_boundary(0, 0, 5)
+    assert e.value.code == TDSE_EINVAL
+    t.close()
+    # dt past the sufficient bound 2 / (6/dx^2 + max|V|)
+    u = make_ctx(8, 8, 8, 1, 0.2, 1.01 * 0.04 / 3.0, "f64")
+    u.set_potential(0, np.zeros((0, 6)), 0.0, 0.0)
+    R0, I0 = random_state(99, (8, 8, 8))
+    u.set_state(0, R0, I0)
+    with pytest.raises(TdseError) as e:
+        u.step(1)
+    assert e.value.code == TDSE_EUNSTABLE
+    u.set_option("allow_unstable", 1)
+    u.step(400)                                   # blow-up just past dt_c = dx^2/3, as the oracle pin
+    R, _ = u.read_psi(0)
+    o = OracleRun(8, 8, 8, 0.2, 1.01 * 0.04 / 3.0, bc=(PERIODIC,) * 3).set_potential_grid(np.zeros((8, 8, 8)))
+    o.set_state(R0, I0).step(400)
+    assert np.linalg.norm(R) / np.linalg.norm(R0) > 1e20
+    assert rel_l2(R, o.R) < 1e-9
+    u.close()
+
+
+def test_three_array_workspace_runs_twopass_only():
+    from paper_2401_07416_b200 import Tdse, TdseError, TDSE_EINVAL
+    w = make_config(0, n=(24, 24, 24), steps=0)
+    t = Tdse.from_workload(w, pingpong=False)
+    assert t.get_info("pingpong") == 0
+    t.step(10)
+    assert t.get_info("kernel") == TWOPASS
+    t.set_option("kernel", FUSED)
+    with pytest.raises(TdseError) as e:
+        t.step(1)
+    assert e.value.code == TDSE_EINVAL
+    R, I = t.read_psi(0)
+    o = OracleRun.from_workload(w).step(10)
+    assert rel_l2(R, o.R) < 1e-12
+    t.close()
+
+
+def test_odd_nx_falls_back_to_twopass_under_auto():
+    from paper_2401_07416_b200 import Tdse
+    w = make_config(1, n=(23, 17, 19), steps=0)
+    t = Tdse.from_workload(w)
+    t.step(12)
+    assert t.get_info("kernel") == TWOPASS
+    R, I = t.read_psi(0)
+    D, tr = t.detector_read(0)
+    o = OracleRun.from_workload(w).step(12)
+    assert rel_l2(R, o.R) < 1e-12 and rel_l2(I, o.I) < 1e-12 and rel_l2(D, o.D) < 1e-12
+    t.close()
+
+
+def test_user_stream_and_device_resident_inputs():
+    import torch
+    from paper_2401_07416_b200 import Tdse
+    w = make_config(3, n=(32, 32, 32), batch=2, steps=0)
+    s = torch.cuda.Stream()
+    t = Tdse(w.nx, w.ny, w.nz, w.batch, w.dx, w.dt, 1.0, 1.0, w.dtype, stream=s)
+    t.set_boundary(*w.bc, w.absorb_lo, w.absorb_hi, w.strength, w.power)
+    dev_atoms = [torch.from_numpy(a).to("cuda") for a in w.atoms]
+    torch.cuda.synchronize()
+    for b in range(w.batch):
+        t.set_potential_device(b, dev_atoms[b], w.atoms[b].shape[0], w.vmin, w.vmax, w.rcut)
+    p = w.packet
+    t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], 0.0)
+    t.set_detector(w.k_det, 10, 4)
+    t.step(40)
+    s.synchronize()
+    img_ptr, tr_ptr, ms = t.detector_device()
+    assert img_ptr and tr_ptr and ms == 4
+    for b in range(w.batch):
+        R, I = t.read_psi(b)
+        D, tr = t.detector_read(b)
+        o = oracle_for(w, b, 40)
+        assert rel_l2(R, o.R) < 1e-4 and rel_l2(D, o.D) < 1e-4 and rel_l2(tr, o.trace) < 1e-4
+    t.close()
