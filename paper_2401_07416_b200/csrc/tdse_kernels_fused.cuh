@@ -278,7 +278,7 @@ fdtd_fused_kernel(const FusedParams P)
             for (int s = 0; s < NS; ++s) { fold[s][j] = fmid[s][j]; fmid[s][j] = fnew[s]; }
 #pragma unroll
             for (int s = NS; s > 2; --s) vq[s][j] = vq[s - 1][j];
-            if (NS > 2) vq[2][j] = dg1;
+            vq[2][j] = dg1;
         }
     }
     cp_async_wait<0>();
