@@ -205,9 +205,11 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm)
 {
     using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
     auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF>;
+    constexpr size_t kMaxSmem = 227 * 1024;
+    static_assert(Tr::SMEM_FIXED + 64 * sizeof(real) <= kMaxSmem, "fused tile does not fit in shared memory");
     static bool attr_set = false;
     if (!attr_set) {
-        CU_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Tr::SMEM_BYTES));
+        CU_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
         attr_set = true;
     }
     P.tiles_x = (c->g.nx + BX - 1) / BX;
@@ -216,21 +218,25 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm)
     // choose the number of z chunks: minimise waves * (chunk length + halo planes)
     const long long slots = (long long)c->num_sms * ctas_per_sm;
     const int H = Tr::H;
-    int best_n = 1;
+    const int max_bz = (int)((kMaxSmem - Tr::SMEM_FIXED) / sizeof(real)) - 2 * H - 2;   // mask table must fit
+    int best_n = 0;
     double best_cost = std::numeric_limits<double>::max();
     const int max_chunks = std::max(1, c->g.nz / std::max(4 * H, 8));
-    for (int n = 1; n <= max_chunks; ++n) {
+    for (int n = 1; n <= std::max(max_chunks, (c->g.nz + max_bz - 1) / max_bz); ++n) {
         const int bz = (c->g.nz + n - 1) / n;
+        if (bz > max_bz) continue;
         const int n_eff = (c->g.nz + bz - 1) / bz;
         const long long waves = (units * n_eff + slots - 1) / slots;
         const double cost = (double)waves * (bz + 2 * H + 3);   // +3: pipeline fill/launch overhead in plane units
         if (cost < best_cost - 1e-9) { best_cost = cost; best_n = n_eff; }
     }
+    if (best_n == 0) return fail(c, TDSE_EINVAL, "fused launch: no feasible z chunking");
     P.bz = (c->g.nz + best_n - 1) / best_n;
     P.nchunks = (c->g.nz + P.bz - 1) / P.bz;
     const long long grid = units * P.nchunks;
     if (grid > 0x7fffffffLL) return fail(c, TDSE_EINVAL, "fused grid too large");
-    kern<<<(unsigned)grid, NT, Tr::SMEM_BYTES, c->stream>>>(P);
+    const size_t smem = Tr::SMEM_FIXED + (size_t)(P.bz + 2 * H + 2) * sizeof(real);
+    kern<<<(unsigned)grid, NT, smem, c->stream>>>(P);
     CU_LAUNCH_CHECK(c);
     c->last_tile_x = BX; c->last_tile_y = BY; c->last_chunks = P.nchunks;
     return TDSE_OK;
@@ -239,17 +245,18 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm)
 int launch_fused(tdse_ctx* c, FusedParams& P, int T)
 {
     if (c->dtype == TDSE_F32) {
-        if (T == 2) return launch_fused_cfg<float, 2, 64, 32, 384, 2>(c, P, 1);
-        return launch_fused_cfg<float, 1, 64, 32, 672, 2>(c, P, 1);
+        if (T == 2) return launch_fused_cfg<float, 2, 64, 32, 384, 1>(c, P, 1);
+        return launch_fused_cfg<float, 1, 64, 32, 672, 1>(c, P, 1);
     }
-    if (T == 2) return launch_fused_cfg<double, 2, 32, 32, 416, 1>(c, P, 1);
-    return launch_fused_cfg<double, 1, 32, 32, 352, 2>(c, P, 1);
+    if (T == 2) return launch_fused_cfg<double, 2, 32, 24, 320, 1>(c, P, 1);
+    return launch_fused_cfg<double, 1, 32, 32, 384, 1>(c, P, 1);
 }
 
 bool fused_supported(const tdse_ctx* c)
 {
     const int vw = (int)(16 / c->w);
-    return c->pingpong && (c->g.nx % vw == 0);
+    // 16-byte vectors along x; per-entry byte offsets are 32-bit inside the fused kernel
+    return c->pingpong && (c->g.nx % vw == 0) && ((unsigned long long)c->g.cells * c->w < (1ull << 32));
 }
 
 template <typename real>
@@ -277,7 +284,7 @@ int finish_trace(tdse_ctx* c, int nparts)
 }
 
 template <typename real>
-int sample_detector_twopass(tdse_ctx* c)
+int sample_detector(tdse_ctx* c)
 {
     const unsigned nblk = (unsigned)((c->g.plane + 255) / 256);
     int rc = ensure_partial(c, (size_t)nblk * c->g.batch);
@@ -573,7 +580,7 @@ int tdse_step(tdse_ctx* c, int n)
             c->steps += 1; remaining -= 1;
             c->last_tblock = 1;
             if (to_sample == 1) {
-                rc = (c->dtype == TDSE_F32) ? sample_detector_twopass<float>(c) : sample_detector_twopass<double>(c);
+                rc = (c->dtype == TDSE_F32) ? sample_detector<float>(c) : sample_detector<double>(c);
                 if (rc) return rc;
             }
         } else {
@@ -586,20 +593,13 @@ int tdse_step(tdse_ctx* c, int n)
             P.nx = c->g.nx; P.ny = c->g.ny; P.nz = c->g.nz; P.batch = c->g.batch;
             P.bcx = c->g.bcx; P.bcy = c->g.bcy; P.bcz = c->g.bcz;
             P.c = c->c; P.cv = c->cv;
-            P.sample = sample ? 1 : 0; P.k_det = c->k_det; P.D = c->D;
-            if (sample) {
-                const size_t max_tiles = (size_t)((c->g.nx + 15) / 16) * ((c->g.ny + 7) / 8);   // tiles are never smaller than 16 x 8
-                rc = ensure_partial(c, (size_t)c->g.batch * max_tiles);
-                if (rc) return rc;
-            }
-            P.partial = c->partial;
             rc = launch_fused(c, P, T);
             if (rc) return rc;
             c->cur ^= 1;
             c->steps += T; remaining -= T;
             c->last_tblock = T;
-            if (sample) {
-                rc = finish_trace(c, P.tiles_x * P.tiles_y);
+            if (sample) {   // R^s and I^{s-1/2} are exactly what the pass just wrote
+                rc = (c->dtype == TDSE_F32) ? sample_detector<float>(c) : sample_detector<double>(c);
                 if (rc) return rc;
             }
         }

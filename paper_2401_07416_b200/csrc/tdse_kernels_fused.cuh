@@ -13,15 +13,17 @@
 //   * planes of R, I, V arrive in a shared-memory ring through cp.async (16 B per thread, zero fill
 //     for Dirichlet ghosts, index wrap for periodic axes resolved once per thread before the march);
 //   * each thread keeps, per stage, the previous two z-planes of its cells in registers (register-rotated
-//     z neighbours); y neighbours come from a double-buffered shared-memory plane per stage, x neighbours
-//     from warp shuffles (lane edges read shared memory);
+//     z neighbours: the march is unrolled by 3 so the rotation costs no moves); y neighbours come from a
+//     double-buffered shared-memory plane per stage, x neighbours from warp shuffles (lane edges read
+//     shared memory);
 //   * all 2T stages of the software pipeline run between two __syncthreads(); stage s works on plane p-s
 //     while plane p+PF is in flight;
-//   * final R and I planes are written with 128-bit stores; on a sampling step the CTAs that own the
-//     detector plane add R^2 + I^2 into the image and produce one partial sum per tile (warp-shuffle
-//     reduction) for the trace.
+//   * halo cells are recomputed, not exchanged: the region shrinks by one cell per stage, and values
+//     outside that shrinking region are garbage that never reaches a cell that is stored.
 // Compulsory HBM traffic: 5 words per cell per launch, i.e. 5/T words per cell-update.
 #pragma once
+#include <type_traits>
+
 #include "tdse_common.cuh"
 
 namespace tdse {
@@ -34,10 +36,6 @@ struct FusedParams {
     int bcx, bcy, bcz;
     int tiles_x, tiles_y, nchunks, bz;                 // z chunk length (last chunk may be shorter)
     double c, cv;
-    int sample;                                        // 1: accumulate detector on plane k_det
-    int k_det;
-    double* D;                                         // [batch][ny][nx]
-    double* partial;                                   // [batch][tiles_x*tiles_y]
 };
 
 __device__ __forceinline__ void cp_async_16(void* smem_dst, const void* gmem_src, int src_bytes)
@@ -61,12 +59,23 @@ struct FusedTraits {
     static constexpr int WQ = W / VW;                          // 16-byte groups per row
     static constexpr int G = WQ * RH;                          // groups per plane
     static constexpr int GPT = (G + NT - 1) / NT;              // groups per thread
-    static constexpr int PLANE = W * RH;                       // elements per staged plane
+    static constexpr int PS = GPT * NT * VW;                   // plane stride in shared memory (padded to whole threads)
+    static constexpr int GUARD = W;                            // one row before the first and after the last plane
     static constexpr int RD = PF + 2;                          // ring depth
-    static constexpr int SMEM_ELEMS = 3 * RD * PLANE + (NS - 1) * 2 * PLANE;
-    static constexpr size_t SMEM_BYTES = (size_t)SMEM_ELEMS * sizeof(real) + 32 * sizeof(double);
+    static constexpr int XD = 3;                               // exchange planes per stage (period of the unrolled march)
+    static constexpr int NPLANES = 3 * RD + (NS - 1) * XD;
+    static constexpr size_t SMEM_FIXED = ((size_t)NPLANES * PS + 2 * GUARD) * sizeof(real);
+    // + (bz + 2H + 2) mask values, added by the launcher
     static_assert(BX % VW == 0, "tile width must be a multiple of the vector width");
     static_assert(NT % 32 == 0, "whole warps");
+    static_assert(T == 1 || T == 2, "queue rotation below is written for T = 1, 2");
+    static_assert(RD == 3, "ring slots are compile-time constants of the 3x unrolled march");
+};
+
+template <typename real, int NS, int GPT>
+struct Queue {                       // one z-plane worth of per-thread pipeline state
+    Pack<real> f[NS][GPT];           // f[s]: field after stage s (s = 0: R as loaded)
+    Pack<real> dg[GPT];              // 6c + c_v V of the plane that entered together with f[0]
 };
 
 template <typename real, int T, int BX, int BY, int NT, int PF>
@@ -75,15 +84,16 @@ fdtd_fused_kernel(const FusedParams P)
 {
     using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
     using V4 = Pack<real>;
-    constexpr int VW = Tr::VW, NS = Tr::NS, H = Tr::H, HX = Tr::HX, WQ = Tr::WQ, RH = Tr::RH;
-    constexpr int G = Tr::G, GPT = Tr::GPT, PLANE = Tr::PLANE, RD = Tr::RD;
+    using Q = Queue<real, Tr::NS, Tr::GPT>;
+    constexpr int VW = Tr::VW, NS = Tr::NS, H = Tr::H, HX = Tr::HX, WQ = Tr::WQ;
+    constexpr int G = Tr::G, GPT = Tr::GPT, PS = Tr::PS, RD = Tr::RD, XD = Tr::XD;
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    real* const ringR = reinterpret_cast<real*>(smem_raw);
-    real* const ringI = ringR + RD * PLANE;
-    real* const ringV = ringI + RD * PLANE;
-    real* const exch = ringV + RD * PLANE;                 // [(NS-1)][2][PLANE], stage s output at exch[(s-1)*2 + parity]
-    double* const scratch = reinterpret_cast<double*>(exch + (NS - 1) * 2 * PLANE);
+    real* const ringR = reinterpret_cast<real*>(smem_raw) + Tr::GUARD;
+    real* const ringI = ringR + RD * PS;
+    real* const ringV = ringI + RD * PS;
+    real* const exch = ringV + RD * PS;                    // stage s output of iteration t at exch[((s-1)*XD + t%3) * PS]
+    real* const smask = exch + (NS - 1) * XD * PS + Tr::GUARD;  // smask[q] = mask of plane Z0-H-1+q
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int ntiles = P.tiles_x * P.tiles_y;
@@ -105,20 +115,18 @@ fdtd_fused_kernel(const FusedParams P)
     const real* __restrict__ gM = static_cast<const real*>(P.mask);
 
     const real c = (real)P.c, cv = (real)P.cv, c6 = (real)(6.0 * P.c);
+    const int soff0 = tid * VW;                      // group j of this thread sits at soff0 + j*NT*VW
+    const int edge_off = (lane == 31) ? VW : -lane * VW - 1;   // see the x-neighbour load in body()
 
     // ---- per-thread geometry, fixed for the whole march ---------------------------------------
     int  goff[GPT];      // offset of the group inside a plane (wrapped), elements
-    int  soff[GPT];      // offset inside a staged plane, elements
-    bool ldok[GPT];      // load from memory (else zero fill: Dirichlet ghost / inactive)
+    bool ldok[GPT];      // load from memory (else zero fill: Dirichlet ghost / padding group)
     bool core[GPT];      // group belongs to the tile's own cells and lies inside the domain
-    int  row[GPT];
 #pragma unroll
     for (int j = 0; j < GPT; ++j) {
         const int g = tid + j * NT;
         const bool act = g < G;
-        const int r = act ? g / WQ : 0, q = act ? g % WQ : 0;
-        row[j] = act ? r : -1000;
-        soff[j] = (act ? g : 0) * VW;
+        const int r = g / WQ, q = g % WQ;
         const int xg = X0 - HX + q * VW, yg = Y0 - H + r;
         bool inx = xg >= 0 && xg < P.nx, iny = yg >= 0 && yg < P.ny;
         int xw = xg, yw = yg;
@@ -135,121 +143,125 @@ fdtd_fused_kernel(const FusedParams P)
         if (P.bcz == BC_PERIODIC) { ok = true; return wrap_index(pz, P.nz); }
         return ok ? pz : 0;
     };
-    auto issue_plane = [&](int t) {                  // stage plane t of the march into ring slot t % RD
-        bool zok;
-        const int pz = zplane(Z0 - H + t, zok);
-        const long long poff = (long long)pz * plane;
-        const int slot = (t % RD) * PLANE;
+    // Byte offsets inside one entry fit 32 bits (the launcher checks cells * sizeof(real) < 4 GiB).
+    const char* const bR = reinterpret_cast<const char*>(gR);
+    const char* const bI = reinterpret_cast<const char*>(gI);
+    const char* const bV = reinterpret_cast<const char*>(gV);
+    const unsigned plane_bytes = (unsigned)plane * (unsigned)sizeof(real);
+    int pz_next;                                     // wrapped index of the next plane to stage
+    {
+        bool ok_unused;
+        pz_next = (P.bcz == BC_PERIODIC) ? zplane(Z0 - H, ok_unused) : Z0 - H;
+    }
+    auto issue_plane = [&](int slot_idx) {           // stage the next plane of the march into ring slot slot_idx
+        const bool zok = (P.bcz == BC_PERIODIC) || (pz_next >= 0 && pz_next < P.nz);
+        const unsigned pb = zok ? (unsigned)pz_next * plane_bytes : 0u;
+        real* dst = ringR + slot_idx * PS + soff0;
 #pragma unroll
         for (int j = 0; j < GPT; ++j) {
-            if (tid + j * NT < G) {
-                const int nbytes = (ldok[j] && zok) ? 16 : 0;
-                const long long o = poff + goff[j];
-                cp_async_16(ringR + slot + soff[j], gR + o, nbytes);
-                cp_async_16(ringI + slot + soff[j], gI + o, nbytes);
-                cp_async_16(ringV + slot + soff[j], gV + o, nbytes);
-            }
+            const int nbytes = (ldok[j] && zok) ? 16 : 0;      // 0: zero fill (ghost cells, padding groups)
+            const unsigned o = pb + (unsigned)goff[j] * (unsigned)sizeof(real);
+            cp_async_16(dst + j * NT * VW, bR + o, nbytes);
+            cp_async_16(dst + RD * PS + j * NT * VW, bI + o, nbytes);
+            cp_async_16(dst + 2 * RD * PS + j * NT * VW, bV + o, nbytes);
         }
+        ++pz_next;
+        if (P.bcz == BC_PERIODIC && pz_next == P.nz) pz_next = 0;
     };
 
-    // ---- register queues ------------------------------------------------------------------------
-    // f[s] (s = 0..NS-1): field after stage s (s = 0: R as loaded).  mid = plane p-s-1, old = plane p-s-2
-    // relative to the plane p that arrives in the current iteration.
-    V4 fmid[NS][GPT], fold[NS][GPT];
-    V4 vq[NS + 1][GPT];      // vq[s] = 6c + c_v V at plane p-s, s = 2..NS (index 0, 1 unused)
-    real mq[NS + 1];         // mq[s] = mask of plane p-s
+    const int niter = bzc + 2 * H;                   // planes Z0-H .. Z0+bzc+H-1 enter the pipeline
+
+    // mask of planes Z0-H-1 .. Z0+bzc+H-1 (0 outside a Dirichlet domain: forces ghost planes to zero)
+    for (int q = tid; q < niter + 1; q += NT) {
+        bool zok;
+        const int pz = zplane(Z0 - H - 1 + q, zok);
+        smask[q] = zok ? gM[pz] : (real)0;
+    }
+    // exchange planes start defined (they are read one iteration before they are first written)
+    for (int q = tid; q < (NS - 1) * XD * PS; q += NT) exch[q] = 0;
+
+    Q qa, qb, qc;
 #pragma unroll
     for (int s = 0; s < NS; ++s)
 #pragma unroll
         for (int j = 0; j < GPT; ++j)
 #pragma unroll
-            for (int e = 0; e < VW; ++e) { fmid[s][j].e[e] = 0; fold[s][j].e[e] = 0; }
+            for (int e = 0; e < VW; ++e) { qa.f[s][j].e[e] = 0; qb.f[s][j].e[e] = 0; qc.f[s][j].e[e] = 0; }
 #pragma unroll
-    for (int s = 0; s <= NS; ++s) {
-        mq[s] = 0;
+    for (int j = 0; j < GPT; ++j)
 #pragma unroll
-        for (int j = 0; j < GPT; ++j)
+        for (int e = 0; e < VW; ++e) { qa.dg[j].e[e] = 0; qb.dg[j].e[e] = 0; qc.dg[j].e[e] = 0; }
+    real mq[NS + 1];
 #pragma unroll
-            for (int e = 0; e < VW; ++e) vq[s][j].e[e] = 0;
-    }
-    // exchange planes start defined (they are read one iteration before they are first written)
-    for (int q = tid; q < (NS - 1) * 2 * PLANE; q += NT) exch[q] = 0;
-
-    double det_sum = 0.0;
-    const int niter = bzc + 2 * H;                   // planes Z0-H .. Z0+bzc+H-1
+    for (int s = 0; s <= NS; ++s) mq[s] = 0;
 
     // ---- prologue: PF planes in flight -----------------------------------------------------------
 #pragma unroll
-    for (int t = 0; t < PF; ++t) { if (t < niter) issue_plane(t); cp_async_commit(); }
+    for (int t = 0; t < PF; ++t) { if (t < niter) issue_plane(t % RD); cp_async_commit(); }
 
-#pragma unroll 1
-    for (int t = 0; t < niter; ++t) {
+    // One iteration of the march: plane p = Z0-H+t has arrived.  `old`/`mid` hold planes p-s-2 / p-s-1 of
+    // every stage s; `nw` receives plane p-s.  (old, mid, nw) rotate by renaming: see the calls below.
+    // `ph` = t % 3 is a compile-time constant of the unrolled march, so every shared-memory offset below is
+    // an immediate relative to one per-thread base register.
+    auto body = [&](const int t, auto phase, Q& old, Q& mid, Q& nw) {
+        constexpr int ph = decltype(phase)::value;
+        constexpr int ph_prev = (ph + 2) % 3;
         cp_async_wait<PF - 1>();
         __syncthreads();
-        if (t + PF < niter) issue_plane(t + PF);
+        if (t + PF < niter) issue_plane((ph + PF) % RD);
         cp_async_commit();
 
-        const int p = Z0 - H + t;                    // global plane that just arrived
-        const int cur = (t % RD) * PLANE;
-        const int prv = ((t + RD - 1) % RD) * PLANE;
-        const int par = t & 1;
-        // mask of plane p-1 enters the queue (0 outside a Dirichlet domain -> forces ghost planes to zero)
+        const int p = Z0 - H + t;
+        const real* curR = ringR + ph * PS + soff0;
+        constexpr int prvo_c = ph_prev * PS;
+        const int prvo = prvo_c + soff0;
 #pragma unroll
         for (int s = NS; s > 1; --s) mq[s] = mq[s - 1];
-        {
-            bool zok;
-            const int pz = zplane(p - 1, zok);
-            mq[1] = zok ? gM[pz] : (real)0;
-        }
+        mq[1] = smask[t];                            // plane p-1
 
 #pragma unroll
         for (int j = 0; j < GPT; ++j) {
-            const bool act = tid + j * NT < G;       // inactive tail groups still take part in the shuffles
-            V4 fnew[NS + 1];
-            fnew[0] = *reinterpret_cast<const V4*>(ringR + cur + soff[j]);
-            const V4 iold = *reinterpret_cast<const V4*>(ringI + prv + soff[j]);
-            const V4 vraw = *reinterpret_cast<const V4*>(ringV + prv + soff[j]);
-            V4 dg1;
+            const int jo = j * NT * VW;
+            V4 dg_oldest;
+            if (NS > 3) dg_oldest = nw.dg[j];        // created three iterations ago: plane p-4
+            nw.f[0][j] = *reinterpret_cast<const V4*>(curR + jo);
+            const V4 iold = *reinterpret_cast<const V4*>(ringI + prvo + jo);
+            const V4 vraw = *reinterpret_cast<const V4*>(ringV + prvo + jo);
 #pragma unroll
-            for (int e = 0; e < VW; ++e) dg1.e[e] = fma(cv, vraw.e[e], c6);
+            for (int e = 0; e < VW; ++e) nw.dg[j].e[e] = fma(cv, vraw.e[e], c6);
 
 #pragma unroll
             for (int s = 1; s <= NS; ++s) {
-                const V4& ctr = fmid[s - 1][j];
-                const V4& zlo = fold[s - 1][j];
-                const V4& zhi = fnew[s - 1];
-                const V4& older = (s == 1) ? iold : fold[s >= 2 ? s - 2 : 0][j];
-                const V4& dg = (s == 1) ? dg1 : vq[s][j];
-                // plane holding the centre values of this stage (written by the previous iteration)
-                const real* cplane = (s == 1) ? (ringR + prv) : (exch + ((s >= 2 ? s - 2 : 0) * 2 + (par ^ 1)) * PLANE);
-                // x neighbours: shuffles inside the warp, shared memory at the warp edges
-                real xm = __shfl_up_sync(0xffffffffu, ctr.e[VW - 1], 1);
-                real xp = __shfl_down_sync(0xffffffffu, ctr.e[0], 1);
-                const bool rowok = row[j] >= s && row[j] < RH - s;
+                const V4& ctr = mid.f[s - 1][j];
+                const V4& zlo = old.f[s - 1][j];
+                const V4& zhi = nw.f[s - 1][j];
+                const V4& older = (s == 1) ? iold : old.f[s >= 2 ? s - 2 : 0][j];
+                const V4& dg = (s == 1) ? nw.dg[j] : (s == 2) ? mid.dg[j] : (s == 3) ? old.dg[j] : dg_oldest;
+                // plane holding the centre values of this stage (written during the previous iteration)
+                const real* cplane = ((s == 1) ? (ringR + prvo) : (exch + ((s >= 2 ? s - 2 : 0) * XD + ph_prev) * PS + soff0)) + jo;
+                // x neighbours: shuffles inside the warp; the two warp-edge lanes take theirs from shared memory
+                // with ONE load per warp (lane 31 reads its right neighbour, all others lane 0's left neighbour)
+                const real edge = cplane[edge_off];
+                const real xm_s = __shfl_up_sync(0xffffffffu, ctr.e[VW - 1], 1);
+                const real xp_s = __shfl_down_sync(0xffffffffu, ctr.e[0], 1);
+                const real xm = (lane == 0) ? edge : xm_s;
+                const real xp = (lane == 31) ? edge : xp_s;
+                const V4 ym = *reinterpret_cast<const V4*>(cplane - WQ * VW);
+                const V4 yp = *reinterpret_cast<const V4*>(cplane + WQ * VW);
+                const real m = ldok[j] ? mq[s] : (real)0;
                 V4 out;
-                if (rowok) {
-                    if (lane == 0) xm = cplane[soff[j] - 1];
-                    if (lane == 31) xp = cplane[soff[j] + VW];
-                    const V4 ym = *reinterpret_cast<const V4*>(cplane + soff[j] - WQ * VW);
-                    const V4 yp = *reinterpret_cast<const V4*>(cplane + soff[j] + WQ * VW);
-                    const real m = ldok[j] ? mq[s] : (real)0;
-                    const real sg = (s & 1) ? (real)1 : (real)-1;
 #pragma unroll
-                    for (int e = 0; e < VW; ++e) {
-                        const real left = (e == 0) ? xm : ctr.e[e - 1];
-                        const real right = (e == VW - 1) ? xp : ctr.e[e + 1];
-                        const real nb = ((left + right) + (ym.e[e] + yp.e[e])) + (zlo.e[e] + zhi.e[e]);
-                        const real upd = fma(c, nb, -dg.e[e] * ctr.e[e]);
-                        out.e[e] = m * fma(sg, upd, older.e[e]);
-                    }
-                } else {
-#pragma unroll
-                    for (int e = 0; e < VW; ++e) out.e[e] = 0;
+                for (int e = 0; e < VW; ++e) {
+                    const real left = (e == 0) ? xm : ctr.e[e - 1];
+                    const real right = (e == VW - 1) ? xp : ctr.e[e + 1];
+                    const real nb = ((left + right) + (ym.e[e] + yp.e[e])) + (zlo.e[e] + zhi.e[e]);
+                    const real upd = fma(c, nb, -dg.e[e] * ctr.e[e]);
+                    out.e[e] = m * ((s & 1) ? older.e[e] + upd : older.e[e] - upd);
                 }
-                fnew[s] = out;
-                if (s < NS && act) *reinterpret_cast<V4*>(exch + ((s - 1) * 2 + par) * PLANE + soff[j]) = out;
-
-                // ---- final stages: write back -----------------------------------------------------
+                if (s < NS) {
+                    nw.f[s][j] = out;
+                    *reinterpret_cast<V4*>(exch + ((s - 1) * XD + ph) * PS + soff0 + jo) = out;
+                }
                 if (s == NS - 1) {                   // I^{n+T-1/2} at plane p-NS+1
                     const int pz = p - (NS - 1);
                     if (core[j] && pz >= Z0 && pz < Z0 + bzc)
@@ -257,36 +269,22 @@ fdtd_fused_kernel(const FusedParams P)
                 }
                 if (s == NS) {                       // R^{n+T} at plane p-NS
                     const int pz = p - NS;
-                    if (core[j] && pz >= Z0 && pz < Z0 + bzc) {
+                    if (core[j] && pz >= Z0 && pz < Z0 + bzc)
                         *reinterpret_cast<V4*>(oR + (long long)pz * plane + goff[j]) = out;
-                        if (P.sample && pz == P.k_det) {
-                            // density of PAPER.md:87: (R^s)^2 + (I^{s-1/2})^2; I at this plane is the centre of stage NS
-                            double* Dp = P.D + (long long)b * plane + goff[j];
-#pragma unroll
-                            for (int e = 0; e < VW; ++e) {
-                                const double r = (double)out.e[e], im = (double)ctr.e[e];
-                                const double rho = r * r + im * im;
-                                Dp[e] += rho;
-                                det_sum += rho;
-                            }
-                        }
-                    }
                 }
             }
-            // ---- rotate the z queues (old <- mid <- new) and the diagonal queue -----------------------
-#pragma unroll
-            for (int s = 0; s < NS; ++s) { fold[s][j] = fmid[s][j]; fmid[s][j] = fnew[s]; }
-#pragma unroll
-            for (int s = NS; s > 2; --s) vq[s][j] = vq[s - 1][j];
-            vq[2][j] = dg1;
         }
+    };
+
+#pragma unroll 1
+    for (int t = 0; t < niter; t += 3) {
+        body(t, std::integral_constant<int, 0>{}, qa, qb, qc);
+        if (t + 1 >= niter) break;
+        body(t + 1, std::integral_constant<int, 1>{}, qb, qc, qa);
+        if (t + 2 >= niter) break;
+        body(t + 2, std::integral_constant<int, 2>{}, qc, qa, qb);
     }
     cp_async_wait<0>();
-
-    if (P.sample && P.k_det >= Z0 && P.k_det < Z0 + bzc) {
-        const double s = block_sum(det_sum, scratch);
-        if (tid == 0) P.partial[(long long)b * ntiles + tile] = s;
-    }
 }
 
 }  // namespace tdse
