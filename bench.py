@@ -204,16 +204,10 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     idx, w = workload_from_args(a, rank)
-    if world > 1 and idx == 3:
-        # weak scaling: every rank generates its own 64 configurations (different seeds), no collective on the data path
-        from workloads.configs import _film_atoms, fcc111_slab
-        lx, ly, lz = w.nx * w.dx, w.ny * w.dx, w.nz * w.dx
-        slab = fcc111_slab(lx, ly, 0.55 * lz, 3)
-        atoms = []
-        for b in range(w.batch):
-            rng = np.random.default_rng(3000 + rank * w.batch + b)
-            atoms.append(np.concatenate([slab, _film_atoms(rng, lx, ly, 0.55 * lz, 12, 0.1, 0.5)], axis=0))
-        w = w.with_(atoms=atoms)
+    if world > 1:
+        # weak scaling: every rank owns its own batch of entries (different seeds), no collective on the data path
+        from workloads import shard_for_rank
+        w = shard_for_rank(w, idx, rank, world)
 
     stream = torch.cuda.Stream()
     t = Tdse(w.nx, w.ny, w.nz, w.batch, w.dx, w.dt, w.mass, w.hbar, w.dtype, stream=stream, device="cuda:%d" % local_rank)

@@ -240,6 +240,40 @@ def make_config(idx: int, *, n: Optional[Sequence[int]] = None, batch: Optional[
     raise ValueError("config index must be 0..4")
 
 
+def shard_for_rank(w: Workload, idx: int, rank: int, world: int) -> Workload:
+    """Weak-scaling shard of configuration `idx` for one rank.
+
+    Entries are independent, so sharding is a partition of entry seeds with no exchange step:
+    rank r owns global entries [r*batch, (r+1)*batch).  For cfg 3 each global entry g has film seed
+    3000 + g; for cfg 2 / cfg 4 the thermal seed is base + g; cfg 0 / cfg 1 have no per-entry
+    randomness (replicas).  rank 0 of any world size reproduces make_config(idx) exactly.
+    """
+    if world < 1 or not (0 <= rank < world):
+        raise ValueError("rank/world")
+    if rank == 0:
+        return w
+    lx, ly, lz = w.nx * w.dx, w.ny * w.dx, w.nz * w.dx
+    g0 = rank * w.batch
+    if idx == 3:
+        z_top = 0.55 * lz
+        slab = fcc111_slab(lx, ly, z_top, 3)
+        atoms, seeds = [], []
+        for b in range(w.batch):
+            seed = 3000 + g0 + b
+            film = _film_atoms(np.random.default_rng(seed), lx, ly, z_top, 12, 0.1, 0.5)
+            atoms.append(np.concatenate([slab, film], axis=0)); seeds.append(seed)
+        return w.with_(atoms=atoms, seeds=seeds)
+    if idx == 2:
+        slab = fcc111_slab(lx, ly, 0.5 * lz, 6)
+        seeds = [2 + g0 + b for b in range(w.batch)]
+        return w.with_(atoms=[_thermal(slab, s) for s in seeds], seeds=seeds)
+    if idx == 4:
+        slab = fcc111_slab(lx, ly, 0.6 * lz, 4)
+        seeds = [4000 + g0 + b for b in range(w.batch)]
+        return w.with_(atoms=[_thermal(slab, s) for s in seeds], seeds=seeds)
+    return w
+
+
 def random_state(seed: int, shape: Sequence[int], dtype=np.float64) -> Tuple[np.ndarray, np.ndarray]:
     """Seeded smooth-free random (R, I_half) pair for raw-state parity cases."""
     rng = np.random.default_rng(seed)
