@@ -69,7 +69,7 @@ struct tdse_ctx {
     double vabs_max = 0.0;
 
     // options / info
-    int opt_kernel = TDSE_KERNEL_AUTO, opt_tblock = 0, allow_unstable = 0;
+    int opt_kernel = TDSE_KERNEL_AUTO, opt_tblock = 0, allow_unstable = 0, opt_pf = 0, opt_chunks = 0;
     long long launches = 0;
     int last_kernel = 0, last_tblock = 0, last_tile_x = 0, last_tile_y = 0, last_chunks = 0;
     int num_sms = 148;
@@ -200,11 +200,11 @@ bool entry_range(const tdse_ctx* c, int b, int* b0, int* b1)
 // ---------------------------------------------------------------------------------------------
 // fused launch table
 // ---------------------------------------------------------------------------------------------
-template <typename real, int T, int BX, int BY, int NT, int PF>
+template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY>
 int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm)
 {
     using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
-    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF>;
+    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF, GHOSTXY>;
     constexpr size_t kMaxSmem = 227 * 1024;
     static_assert(Tr::SMEM_FIXED + 64 * sizeof(real) <= kMaxSmem, "fused tile does not fit in shared memory");
     static bool attr_set = false;
@@ -222,9 +222,10 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm)
     int best_n = 0;
     double best_cost = std::numeric_limits<double>::max();
     const int max_chunks = std::max(1, c->g.nz / std::max(4 * H, 8));
-    for (int n = 1; n <= std::max(max_chunks, (c->g.nz + max_bz - 1) / max_bz); ++n) {
+    for (int n = 1; n <= std::max(std::max(max_chunks, c->opt_chunks), (c->g.nz + max_bz - 1) / max_bz); ++n) {
         const int bz = (c->g.nz + n - 1) / n;
         if (bz > max_bz) continue;
+        if (c->opt_chunks > 0 && n != std::min(c->opt_chunks, c->g.nz)) continue;
         const int n_eff = (c->g.nz + bz - 1) / bz;
         const long long waves = (units * n_eff + slots - 1) / slots;
         const double cost = (double)waves * (bz + 2 * H + 3);   // +3: pipeline fill/launch overhead in plane units
@@ -242,14 +243,30 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm)
     return TDSE_OK;
 }
 
-int launch_fused(tdse_ctx* c, FusedParams& P, int T)
+template <bool GHOSTXY>
+int launch_fused_bc(tdse_ctx* c, FusedParams& P, int T)
 {
     if (c->dtype == TDSE_F32) {
-        if (T == 2) return launch_fused_cfg<float, 2, 64, 32, 384, 1>(c, P, 1);
-        return launch_fused_cfg<float, 1, 64, 32, 672, 1>(c, P, 1);
+        if (T == 2) return c->opt_pf == 1 ? launch_fused_cfg<float, 2, 64, 32, 384, 1, GHOSTXY>(c, P, 1)
+                                          : launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY>(c, P, 1);
+        return c->opt_pf == 1 ? launch_fused_cfg<float, 1, 64, 32, 352, 1, GHOSTXY>(c, P, 1)
+             : c->opt_pf == 2 ? launch_fused_cfg<float, 1, 64, 32, 352, 2, GHOSTXY>(c, P, 1)
+                              : launch_fused_cfg<float, 1, 64, 32, 352, 4, GHOSTXY>(c, P, 1);
     }
-    if (T == 2) return launch_fused_cfg<double, 2, 32, 24, 320, 1>(c, P, 1);
-    return launch_fused_cfg<double, 1, 32, 32, 384, 1>(c, P, 1);
+    if (T == 2) return c->opt_pf == 1 ? launch_fused_cfg<double, 2, 32, 24, 320, 1, GHOSTXY>(c, P, 1)
+                     : c->opt_pf == 2 ? launch_fused_cfg<double, 2, 32, 24, 320, 2, GHOSTXY>(c, P, 1)
+                                      : launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY>(c, P, 1);
+    return c->opt_pf == 1 ? launch_fused_cfg<double, 1, 32, 32, 352, 1, GHOSTXY>(c, P, 1)
+         : c->opt_pf == 2 ? launch_fused_cfg<double, 1, 32, 32, 352, 2, GHOSTXY>(c, P, 1)
+                          : launch_fused_cfg<double, 1, 32, 32, 352, 4, GHOSTXY>(c, P, 1);
+}
+
+int launch_fused(tdse_ctx* c, FusedParams& P, int T)
+{
+    P.cf = (float)P.c; P.cvf = (float)P.cv; P.c6f = (float)(6.0 * P.c);
+    P.entry_bytes = (unsigned long long)c->g.cells * c->w;
+    const bool ghostxy = c->g.bcx == BC_DIRICHLET || c->g.bcy == BC_DIRICHLET;
+    return ghostxy ? launch_fused_bc<true>(c, P, T) : launch_fused_bc<false>(c, P, T);
 }
 
 bool fused_supported(const tdse_ctx* c)
@@ -689,6 +706,12 @@ int tdse_set_option(tdse_ctx* c, const char* key, long long value)
     } else if (k == "tblock") {
         if (value < 0 || value > 2) return fail(c, TDSE_EINVAL, "tdse_set_option: tblock must be 0..2");
         c->opt_tblock = (int)value;
+    } else if (k == "prefetch") {
+        if (value < 0 || value > 4) return fail(c, TDSE_EINVAL, "tdse_set_option: prefetch must be 0..4");
+        c->opt_pf = (int)value;
+    } else if (k == "z_chunks") {
+        if (value < 0) return fail(c, TDSE_EINVAL, "tdse_set_option: z_chunks must be >= 0");
+        c->opt_chunks = (int)value;
     } else if (k == "allow_unstable") {
         c->allow_unstable = value ? 1 : 0;
     } else {
