@@ -55,7 +55,9 @@ typedef struct { double x, y, z, Z, soft2, screen; } tdse_atom;
 enum {
     TDSE_KERNEL_AUTO = 0,     /* fused where the shape allows it, else two-pass */
     TDSE_KERNEL_TWOPASS = 1,  /* one thread per cell, eq (9) launch then eq (8) launch, in place */
-    TDSE_KERNEL_FUSED = 2     /* z-marching fused R+I kernel, T full steps per pass (needs ping-pong) */
+    TDSE_KERNEL_FUSED = 2     /* z-marching fused R+I kernel, T full steps per pass.  Needs the 5-array (ping-pong)
+                               * workspace, nx*sizeof(element) a multiple of 16, even ny, nx >= 8, ny >= 8;
+                               * tdse_step returns TDSE_EINVAL if it is forced on anything else. */
 };
 
 /* Create a context for `batch` independent nx*ny*nz grids with cubic cells of edge dx, time step dt,
@@ -69,7 +71,11 @@ int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
 int tdse_destroy(tdse_ctx* ctx);
 
 /* Bytes of device workspace for the R, I, V grids (pingpong = 0: 3 arrays, two-pass kernels only;
- * pingpong = 1: 5 arrays, needed by the fused kernels).  Returns 0 on invalid arguments. */
+ * pingpong = 1: 5 arrays, needed by the fused kernels).  Inside the workspace every xy plane is stored
+ * with a frame of 4 columns and 4 rows on each side (periodic images or Dirichlet zeros, which lets the
+ * fused kernel fetch tile + halo with one TMA box): one array holds batch*nz*(ny+8)*(nx+8) elements,
+ * rounded up to 256 bytes.  The layout is private to the library; every buffer that crosses this ABI
+ * is the plain [z][y][x] grid.  Returns 0 on invalid arguments. */
 size_t tdse_workspace_bytes(int nx, int ny, int nz, int batch, int dtype, int pingpong);
 
 /* Use caller-owned device memory (e.g. a torch tensor) and a caller-owned CUDA stream (a cudaStream_t

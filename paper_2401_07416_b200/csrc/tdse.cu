@@ -2,6 +2,7 @@
 // sm_100a only.  No CPU fallback: every entry point fails with TDSE_ECUDA without a device.
 #include "../../include/tdse.h"
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -9,6 +10,7 @@
 #include <cstdio>
 #include <cstring>
 #include <limits>
+#include <map>
 #include <new>
 #include <string>
 #include <vector>
@@ -73,6 +75,7 @@ struct tdse_ctx {
     long long launches = 0;
     int last_kernel = 0, last_tblock = 0, last_tile_x = 0, last_tile_y = 0, last_chunks = 0;
     int num_sms = 148;
+    std::map<int, std::vector<CUtensorMap>> tmaps;   // per fused variant: maps of R[0], I[0], V, R[1], I[1]
     std::string err;
 };
 
@@ -114,6 +117,7 @@ void carve(tdse_ctx* c)
         c->R[1] = c->I[1] = nullptr;
     }
     c->cur = 0;
+    c->tmaps.clear();
     std::fill(c->have_V.begin(), c->have_V.end(), 0);
     std::fill(c->have_state.begin(), c->have_state.end(), 0);
     c->vabs_max = 0.0;
@@ -131,6 +135,7 @@ int ensure_workspace(tdse_ctx* c)
     }
     c->ws = p; c->ws_bytes = bytes; c->ws_owned = true; c->pingpong = true;
     carve(c);
+    CU_TRY(c, cudaMemsetAsync(c->ws, 0, bytes, c->stream));   // frames of Dirichlet axes stay zero
     return TDSE_OK;
 }
 
@@ -187,7 +192,31 @@ int reset_detector(tdse_ctx* c)
     return TDSE_OK;
 }
 
-inline char* entry_ptr(const tdse_ctx* c, void* arr, int b) { return static_cast<char*>(arr) + (size_t)b * c->g.cells * c->w; }
+inline char* entry_ptr(const tdse_ctx* c, void* arr, int b) { return static_cast<char*>(arr) + (size_t)b * c->g.pcells * c->w; }
+
+// Copy one entry between a flat [nz][ny][nx] buffer (C-ABI layout) and the framed device storage.
+int copy_entry(tdse_ctx* c, void* dev_entry, void* flat, cudaMemcpyKind kind, bool to_device)
+{
+    cudaMemcpy3DParms p{};
+    const cudaPitchedPtr framed = make_cudaPitchedPtr(dev_entry, (size_t)c->g.px * c->w, (size_t)c->g.px * c->w, (size_t)c->g.py);
+    const cudaPitchedPtr plain = make_cudaPitchedPtr(flat, (size_t)c->g.nx * c->w, (size_t)c->g.nx * c->w, (size_t)c->g.ny);
+    const cudaPos inner = make_cudaPos((size_t)PADX * c->w, (size_t)PADY, 0), origin = make_cudaPos(0, 0, 0);
+    if (to_device) { p.srcPtr = plain; p.srcPos = origin; p.dstPtr = framed; p.dstPos = inner; }
+    else           { p.srcPtr = framed; p.srcPos = inner; p.dstPtr = plain; p.dstPos = origin; }
+    p.extent = make_cudaExtent((size_t)c->g.nx * c->w, (size_t)c->g.ny, (size_t)c->g.nz);
+    p.kind = kind;
+    CU_TRY(c, cudaMemcpy3DAsync(&p, c->stream));
+    return TDSE_OK;
+}
+
+int fill_frame(tdse_ctx* c, void* dev_entry)
+{
+    const unsigned nblk = (unsigned)((c->g.pcells + 255) / 256);
+    if (c->dtype == TDSE_F32) frame_fill_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, static_cast<float*>(dev_entry));
+    else frame_fill_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, static_cast<double*>(dev_entry));
+    CU_LAUNCH_CHECK(c);
+    return TDSE_OK;
+}
 
 bool entry_range(const tdse_ctx* c, int b, int* b0, int* b1)
 {
@@ -195,6 +224,56 @@ bool entry_range(const tdse_ctx* c, int b, int* b0, int* b1)
     if (b < 0 || b >= c->g.batch) return false;
     *b0 = b; *b1 = b + 1;
     return true;
+}
+
+// ---------------------------------------------------------------------------------------------
+// TMA descriptors for the fused kernel: the 5-d view (x, row parity, row pair, z, entry) of one framed
+// array, box = one half-plane of a tile (W x 1 x NP x 1 x 1).  cuTensorMapEncodeTiled is taken from the
+// driver through the runtime (no link against libcuda).
+// ---------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+// maps of R[0], I[0], V, R[1], I[1] for boxes of W columns x NP row pairs
+int get_tensor_maps(tdse_ctx* c, int W, int NP, const CUtensorMap** out)
+{
+    const int key = W * 1024 + NP;
+    auto it = c->tmaps.find(key);
+    if (it == c->tmaps.end()) {
+        EncodeTiledFn enc = encode_tiled_fn();
+        if (!enc) return fail(c, TDSE_ECUDA, "fused launch: cuTensorMapEncodeTiled is not available from the driver");
+        std::vector<CUtensorMap> maps(5);
+        void* arrs[5] = {c->R[0], c->I[0], c->V, c->R[1], c->I[1]};
+        const cuuint64_t w = c->w, px = (cuuint64_t)c->g.px, py = (cuuint64_t)c->g.py;
+        const cuuint64_t dims[5] = {px, 2, py / 2, (cuuint64_t)c->g.nz, (cuuint64_t)c->g.batch};
+        const cuuint64_t strides[4] = {px * w, 2 * px * w, px * py * w, px * py * (cuuint64_t)c->g.nz * w};
+        const cuuint32_t box[5] = {(cuuint32_t)W, 1, (cuuint32_t)NP, 1, 1};
+        const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+        for (int a = 0; a < 5; ++a) {
+            const CUresult r = enc(&maps[a], c->dtype == TDSE_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64,
+                                   5, arrs[a], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                   CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS) return fail(c, TDSE_ECUDA, "fused launch: cuTensorMapEncodeTiled failed with code " + std::to_string((int)r));
+        }
+        it = c->tmaps.emplace(key, std::move(maps)).first;
+    }
+    *out = it->second.data();
+    return TDSE_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -237,7 +316,11 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm)
     const long long grid = units * P.nchunks;
     if (grid > 0x7fffffffLL) return fail(c, TDSE_EINVAL, "fused grid too large");
     const size_t smem = Tr::SMEM_FIXED + (size_t)(P.bz + 2 * H + 2) * sizeof(real);
-    kern<<<(unsigned)grid, NT, smem, c->stream>>>(P);
+    const CUtensorMap* maps = nullptr;
+    int rc = get_tensor_maps(c, Tr::W, Tr::NP, &maps);
+    if (rc) return rc;
+    const int in = c->cur;                              // maps: R[0], I[0], V, R[1], I[1]
+    kern<<<(unsigned)grid, NT, smem, c->stream>>>(P, maps[in ? 3 : 0], maps[in ? 4 : 1], maps[2]);
     CU_LAUNCH_CHECK(c);
     c->last_tile_x = BX; c->last_tile_y = BY; c->last_chunks = P.nchunks;
     return TDSE_OK;
@@ -264,7 +347,8 @@ int launch_fused_bc(tdse_ctx* c, FusedParams& P, int T)
 int launch_fused(tdse_ctx* c, FusedParams& P, int T)
 {
     P.cf = (float)P.c; P.cvf = (float)P.cv; P.c6f = (float)(6.0 * P.c);
-    P.entry_bytes = (unsigned long long)c->g.cells * c->w;
+    P.entry_bytes = (unsigned long long)c->g.pcells * c->w;
+    P.px = c->g.px; P.py = c->g.py;
     const bool ghostxy = c->g.bcx == BC_DIRICHLET || c->g.bcy == BC_DIRICHLET;
     return ghostxy ? launch_fused_bc<true>(c, P, T) : launch_fused_bc<false>(c, P, T);
 }
@@ -273,7 +357,9 @@ bool fused_supported(const tdse_ctx* c)
 {
     const int vw = (int)(16 / c->w);
     // 16-byte vectors along x; per-entry byte offsets are 32-bit inside the fused kernel
-    return c->pingpong && (c->g.nx % vw == 0) && ((unsigned long long)c->g.cells * c->w < (1ull << 32));
+    // (also: even ny for the row-pair view, a domain at least as wide as the frame so that images are first images)
+    return c->pingpong && (c->g.nx % vw == 0) && (c->g.ny % 2 == 0) && c->g.nx >= 2 * PADX && c->g.ny >= 2 * PADY &&
+           ((unsigned long long)c->g.pcells * c->w < (1ull << 32));
 }
 
 template <typename real>
@@ -324,7 +410,7 @@ const char* tdse_last_error(const tdse_ctx* ctx) { return ctx ? ctx->err.c_str()
 size_t tdse_workspace_bytes(int nx, int ny, int nz, int batch, int dtype, int pingpong)
 {
     if (nx < 1 || ny < 1 || nz < 1 || batch < 1 || (dtype != TDSE_F32 && dtype != TDSE_F64)) return 0;
-    const size_t arr = align_up((size_t)nx * ny * nz * batch * elem_bytes(dtype));
+    const size_t arr = align_up((size_t)(nx + 2 * PADX) * (ny + 2 * PADY) * nz * batch * elem_bytes(dtype));
     return (pingpong ? 5 : 3) * arr;
 }
 
@@ -348,11 +434,14 @@ int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
     c->g.bcx = c->g.bcy = c->g.bcz = BC_PERIODIC;
     c->g.plane = (long long)nx * ny;
     c->g.cells = c->g.plane * nz;
+    c->g.px = nx + 2 * PADX; c->g.py = ny + 2 * PADY;
+    c->g.pplane = (long long)c->g.px * c->g.py;
+    c->g.pcells = c->g.pplane * nz;
     c->dtype = dtype; c->w = elem_bytes(dtype);
     c->dx = dx; c->dt = dt; c->mass = mass; c->hbar = hbar;
     c->c = hbar * dt / (2.0 * mass * dx * dx);
     c->cv = dt / hbar;
-    c->arr_bytes = align_up((size_t)c->g.cells * batch * c->w);
+    c->arr_bytes = align_up((size_t)c->g.pcells * batch * c->w);
     c->have_V.assign(batch, 0);
     c->have_state.assign(batch, 0);
     int dev = 0;
@@ -404,6 +493,7 @@ int tdse_bind(tdse_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream)
     c->pingpong = bytes >= 5 * c->arr_bytes;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     carve(c);
+    CU_TRY(c, cudaMemsetAsync(c->ws, 0, (c->pingpong ? 5 : 3) * c->arr_bytes, c->stream));   // frames of Dirichlet axes stay zero
     return reset_detector(c);
 }
 
@@ -431,7 +521,7 @@ static int build_potential(tdse_ctx* c, int b, const AtomRec* atoms_dev, int nat
         potential_build_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->dx, atoms_dev, natoms, vmin, vmax, rcut, static_cast<double*>(dst));
     CU_LAUNCH_CHECK(c);
     for (int e = b0 + 1; e < b1; ++e)
-        CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->V, e), dst, (size_t)c->g.cells * c->w, cudaMemcpyDeviceToDevice, c->stream));
+        CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->V, e), dst, (size_t)c->g.pcells * c->w, cudaMemcpyDeviceToDevice, c->stream));
     for (int e = b0; e < b1; ++e) c->have_V[e] = 1;
     c->vabs_max = std::max(c->vabs_max, std::max(std::fabs(vmin), std::fabs(vmax)));
     return TDSE_OK;
@@ -486,18 +576,20 @@ int tdse_set_potential_grid(tdse_ctx* c, int b, const void* V, int on_device)
     if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_potential_grid: entry out of range");
     int rc = ensure_workspace(c);
     if (rc) return rc;
-    const size_t nbytes = (size_t)c->g.cells * c->w;
     for (int e = b0; e < b1; ++e) {
-        CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->V, e), V, nbytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+        rc = copy_entry(c, entry_ptr(c, c->V, e), const_cast<void*>(V), on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, true);
+        if (rc) return rc;
+        rc = fill_frame(c, entry_ptr(c, c->V, e));
+        if (rc) return rc;
         c->have_V[e] = 1;
     }
     // max |V| for the stability bound
     rc = ensure_partial(c, 1024);
     if (rc) return rc;
     if (c->dtype == TDSE_F32)
-        absmax_partial_kernel<float><<<256, 256, 0, c->stream>>>(static_cast<const float*>((void*)entry_ptr(c, c->V, b0)), c->g.cells, c->partial);
+        absmax_partial_kernel<float><<<256, 256, 0, c->stream>>>(static_cast<const float*>((void*)entry_ptr(c, c->V, b0)), c->g.pcells, c->partial);
     else
-        absmax_partial_kernel<double><<<256, 256, 0, c->stream>>>(static_cast<const double*>((void*)entry_ptr(c, c->V, b0)), c->g.cells, c->partial);
+        absmax_partial_kernel<double><<<256, 256, 0, c->stream>>>(static_cast<const double*>((void*)entry_ptr(c, c->V, b0)), c->g.pcells, c->partial);
     CU_LAUNCH_CHECK(c);
     double part[256];
     CU_TRY(c, cudaMemcpyAsync(part, c->partial, sizeof(part), cudaMemcpyDeviceToHost, c->stream));
@@ -543,11 +635,12 @@ int tdse_set_state(tdse_ctx* c, int b, const void* R, const void* I_half, int on
     if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_state: entry out of range");
     int rc = ensure_workspace(c);
     if (rc) return rc;
-    const size_t nbytes = (size_t)c->g.cells * c->w;
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     for (int e = b0; e < b1; ++e) {
-        CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->R[c->cur], e), R, nbytes, kind, c->stream));
-        CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->I[c->cur], e), I_half, nbytes, kind, c->stream));
+        if ((rc = copy_entry(c, entry_ptr(c, c->R[c->cur], e), const_cast<void*>(R), kind, true))) return rc;
+        if ((rc = copy_entry(c, entry_ptr(c, c->I[c->cur], e), const_cast<void*>(I_half), kind, true))) return rc;
+        if ((rc = fill_frame(c, entry_ptr(c, c->R[c->cur], e)))) return rc;
+        if ((rc = fill_frame(c, entry_ptr(c, c->I[c->cur], e)))) return rc;
         c->have_state[e] = 1;
     }
     if (!on_device) CU_TRY(c, cudaStreamSynchronize(c->stream));   // caller may reuse pageable buffers
@@ -584,7 +677,7 @@ int tdse_step(tdse_ctx* c, int n)
     int kernel = c->opt_kernel;
     if (kernel == TDSE_KERNEL_AUTO) kernel = fused_supported(c) ? TDSE_KERNEL_FUSED : TDSE_KERNEL_TWOPASS;
     if (kernel == TDSE_KERNEL_FUSED && !fused_supported(c))
-        return fail(c, TDSE_EINVAL, "tdse_step: fused kernel needs a 5-array workspace and nx divisible by 16 bytes / element size");
+        return fail(c, TDSE_EINVAL, "tdse_step: fused kernel needs a 5-array workspace, rows of whole 16-byte groups, even ny, nx >= 8 and ny >= 8");
     const int tmax = (c->opt_tblock > 0) ? c->opt_tblock : 2;
     c->last_kernel = kernel;
     int remaining = n;
@@ -653,9 +746,9 @@ int tdse_read_psi(tdse_ctx* c, int b, void* R_host, void* I_host)
     if (!c) return TDSE_EINVAL;
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_read_psi: entry out of range");
     if (!c->ws || !c->have_state[b]) return fail(c, TDSE_ESTATE, "tdse_read_psi: state not set");
-    const size_t nbytes = (size_t)c->g.cells * c->w;
-    if (R_host) CU_TRY(c, cudaMemcpyAsync(R_host, entry_ptr(c, c->R[c->cur], b), nbytes, cudaMemcpyDeviceToHost, c->stream));
-    if (I_host) CU_TRY(c, cudaMemcpyAsync(I_host, entry_ptr(c, c->I[c->cur], b), nbytes, cudaMemcpyDeviceToHost, c->stream));
+    int rc;
+    if (R_host && (rc = copy_entry(c, entry_ptr(c, c->R[c->cur], b), R_host, cudaMemcpyDeviceToHost, false))) return rc;
+    if (I_host && (rc = copy_entry(c, entry_ptr(c, c->I[c->cur], b), I_host, cudaMemcpyDeviceToHost, false))) return rc;
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     return TDSE_OK;
 }
@@ -666,7 +759,7 @@ int tdse_read_potential(tdse_ctx* c, int b, void* V_host)
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_read_potential: entry out of range");
     if (!c->ws || !c->have_V[b]) return fail(c, TDSE_ESTATE, "tdse_read_potential: potential not set");
     if (!V_host) return fail(c, TDSE_EINVAL, "tdse_read_potential: NULL");
-    CU_TRY(c, cudaMemcpyAsync(V_host, entry_ptr(c, c->V, b), (size_t)c->g.cells * c->w, cudaMemcpyDeviceToHost, c->stream));
+    { int rc = copy_entry(c, entry_ptr(c, c->V, b), V_host, cudaMemcpyDeviceToHost, false); if (rc) return rc; }
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     return TDSE_OK;
 }

@@ -57,7 +57,7 @@ potential_build_kernel(Grid g, double dx, const AtomRec* __restrict__ atoms, int
     }
     if (live) {
         sum = fmin(fmax(sum, vmin), vmax);
-        V[cell] = (real)sum;
+        store_with_images(V, g, i, j, k, (real)sum);
     }
 }
 
@@ -108,9 +108,9 @@ wavepacket_init_kernel(Grid g, double dx, PacketParams p, double c, double cv,
     const double d2x = packet_re_nbr(p, g, dx, i + 1, j, k) - 2.0 * re + packet_re_nbr(p, g, dx, i - 1, j, k);
     const double d2y = packet_re_nbr(p, g, dx, i, j + 1, k) - 2.0 * re + packet_re_nbr(p, g, dx, i, j - 1, k);
     const double d2z = packet_re_nbr(p, g, dx, i, j, k + 1) - 2.0 * re + packet_re_nbr(p, g, dx, i, j, k - 1);
-    const double Ar = -c * d2x - c * d2y - c * d2z + cv * (double)V[cell] * re;
-    R[cell] = (real)re;
-    I[cell] = (real)(im + 0.5 * Ar);
+    const double Ar = -c * d2x - c * d2y - c * d2z + cv * (double)V[cell_offset(g, i, j, k)] * re;
+    store_with_images(R, g, i, j, k, (real)re);
+    store_with_images(I, g, i, j, k, (real)(im + 0.5 * Ar));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -129,7 +129,7 @@ __device__ __forceinline__ real load_nbr(const real* __restrict__ f, const Grid&
     if (j >= g.ny) { if (g.bcy == BC_PERIODIC) j = 0;        else return (real)0; }
     if (k < 0)     { if (g.bcz == BC_PERIODIC) k = g.nz - 1; else return (real)0; }
     if (k >= g.nz) { if (g.bcz == BC_PERIODIC) k = 0;        else return (real)0; }
-    return f[((long long)k * g.ny + j) * g.nx + i];
+    return f[cell_offset(g, i, j, k)];
 }
 
 template <typename real>
@@ -140,19 +140,20 @@ half_step_kernel(Grid g, real c, real cv, real sgn, const real* __restrict__ V,
     // grid: x = cells of one entry / 256, y = batch entry
     const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (cell >= g.cells) return;
-    const long long base = (long long)blockIdx.y * g.cells;
+    const long long base = (long long)blockIdx.y * g.pcells;
     const int i = (int)(cell % g.nx);
     const long long t = cell / g.nx;
     const int j = (int)(t % g.ny);
     const int k = (int)(t / g.ny);
     const real* s = src + base;
-    const real s0 = s[cell];
+    const long long o = cell_offset(g, i, j, k);
+    const real s0 = s[o];
     const real nb = (load_nbr(s, g, i + 1, j, k) + load_nbr(s, g, i - 1, j, k))
                   + (load_nbr(s, g, i, j + 1, k) + load_nbr(s, g, i, j - 1, k))
                   + (load_nbr(s, g, i, j, k + 1) + load_nbr(s, g, i, j, k - 1));
     const real lap = nb - (real)6 * s0;
-    const real upd = c * lap - cv * V[base + cell] * s0;
-    dst[base + cell] = M[k] * (dst[base + cell] + sgn * upd);
+    const real upd = c * lap - cv * V[base + o] * s0;
+    store_with_images(dst + base, g, i, j, k, M[k] * (dst[base + o] + sgn * upd));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -169,7 +170,7 @@ detector_accum_kernel(Grid g, int k_det, const real* __restrict__ R, const real*
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     double rho = 0.0;
     if (p < g.plane) {
-        const long long off = (long long)blockIdx.y * g.cells + (long long)k_det * g.plane + p;
+        const long long off = (long long)blockIdx.y * g.pcells + cell_offset(g, (int)(p % g.nx), (int)(p / g.nx), k_det);
         const double r = (double)R[off], im = (double)I[off];
         rho = r * r + im * im;
         D[(long long)blockIdx.y * g.plane + p] += rho;
@@ -206,11 +207,12 @@ norm_partial_kernel(Grid g, double c, double cv, const real* __restrict__ V, con
         const long long t = cell / g.nx;
         const int j = (int)(t % g.ny);
         const int k = (int)(t / g.ny);
-        const double r0 = (double)R[cell], i0 = (double)I[cell];
+        const long long o = cell_offset(g, i, j, k);
+        const double r0 = (double)R[o], i0 = (double)I[o];
         const double nb = ((double)load_nbr(R, g, i + 1, j, k) + (double)load_nbr(R, g, i - 1, j, k))
                         + ((double)load_nbr(R, g, i, j + 1, k) + (double)load_nbr(R, g, i, j - 1, k))
                         + ((double)load_nbr(R, g, i, j, k + 1) + (double)load_nbr(R, g, i, j, k - 1));
-        const double ip = (double)M[k] * (i0 + c * (nb - 6.0 * r0) - cv * (double)V[cell] * r0);
+        const double ip = (double)M[k] * (i0 + c * (nb - 6.0 * r0) - cv * (double)V[o] * r0);
         qv = r0 * r0 + ip * i0;
         qp = r0 * r0 + i0 * i0;
     }
@@ -235,7 +237,26 @@ reduce_rows_kernel(const double* __restrict__ partial, int n, int rows, double s
     }
 }
 
-// max |V| over one entry (for the stability bound after a raw-grid upload).
+// Fill the frame of one entry's array with the periodic images of the interior (after a raw upload).
+// One thread per stored element of the entry; Dirichlet axes keep their zero frame.
+template <typename real>
+__global__ void __launch_bounds__(256)
+frame_fill_kernel(Grid g, real* __restrict__ f)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= g.pcells) return;
+    const int xi = (int)(e % g.px) - PADX;
+    const long long t = e / g.px;
+    const int yj = (int)(t % g.py) - PADY;
+    const int k = (int)(t / g.py);
+    const bool fx = xi < 0 || xi >= g.nx, fy = yj < 0 || yj >= g.ny;
+    if (!fx && !fy) return;
+    if ((fx && g.bcx != BC_PERIODIC) || (fy && g.bcy != BC_PERIODIC)) { f[e] = (real)0; return; }
+    f[e] = f[cell_offset(g, wrap_index(xi, g.nx), wrap_index(yj, g.ny), k)];
+}
+
+// max |V| over one entry (for the stability bound after a raw-grid upload).  The frame holds images or zeros,
+// so scanning the stored elements gives the same maximum.
 template <typename real>
 __global__ void __launch_bounds__(256)
 absmax_partial_kernel(const real* __restrict__ V, long long n, double* __restrict__ partial)

@@ -10,19 +10,27 @@
 // Design (differs from the paper's one-thread-per-point kernel, on purpose):
 //   * a CTA owns an xy tile (BX x BY cells + halo of 2T) of one batch entry and marches a z chunk;
 //     ping-pong buffers (Rin,Iin -> Rout,Iout) make neighbouring tiles independent;
-//   * planes of R, I, V arrive in a shared-memory ring through cp.async (16 B per thread, zero fill
-//     for Dirichlet ghosts, index wrap for periodic axes resolved once per thread before the march);
+//   * planes of R, I, V (tile + halo) arrive in a shared-memory ring through TMA (cp.async.bulk.tensor, one
+//     elected thread, mbarrier completion, PF planes ahead).  Device storage carries a frame of periodic
+//     images / Dirichlet zeros around every xy plane (tdse_common.cuh), so a box never wraps in x or y;
+//     out-of-range z planes (Dirichlet ghosts) are zero-filled by the TMA unit, periodic z wraps the plane
+//     index.  The 5-d tensor view (x, row parity, row pair, z, entry) splits even and odd rows into two
+//     half-planes so that every 16-byte shared-memory access of a warp is contiguous (no bank conflicts);
 //   * a thread owns a 2-row x 16-byte patch of the tile (rows 2rp, 2rp+1).  Per stage it keeps the previous
 //     two z-planes of its cells in registers (register-rotated z neighbours: the march is unrolled by 3 so
 //     the rotation costs no moves); the y neighbour between its two rows is a register, the outer two y
 //     neighbours come from the stage's shared-memory exchange plane, x neighbours from warp shuffles (the
 //     two warp-edge lanes read shared memory);
 //   * all 2T stages of the software pipeline run between two __syncthreads(); stage s works on plane p-s
-//     while plane p+1 is in flight;
+//     while planes p+1 .. p+PF are in flight;
+//   * cells of the tile next to a periodic face are stored twice (corner cells four times): once in place and
+//     once as the image inside the frame, which is what the neighbouring tile's box reads in the next launch;
 //   * halo cells are recomputed, not exchanged: the region shrinks by one cell per stage, and values
 //     outside that shrinking region are garbage that never reaches a cell that is stored.
 // Compulsory HBM traffic: 5 words per cell per launch, i.e. 5/T words per cell-update.
 #pragma once
+#include <cuda.h>
+
 #include <type_traits>
 
 #include "tdse_common.cuh"
@@ -35,20 +43,42 @@ struct FusedParams {
     const void* mask;                                  // real[nz]
     int nx, ny, nz, batch;
     int bcx, bcy, bcz;
+    int px, py;                                        // framed row length / rows per plane
     int tiles_x, tiles_y, nchunks, bz;                 // z chunk length (last chunk may be shorter)
     double c, cv;
     float cf, cvf, c6f;                                // the same, rounded once on the host for float contexts
-    unsigned long long entry_bytes;                    // nx*ny*nz*sizeof(real)
+    unsigned long long entry_bytes;                    // px*py*nz*sizeof(real)
 };
 
-__device__ __forceinline__ void cp_async_16(void* smem_dst, const void* gmem_src, int src_bytes)
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count)
 {
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem_src), "r"(src_bytes) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// one half-plane box (W x 1 x NP x 1 x 1) of the 5-d view (x, row parity, row pair, z, entry)
+__device__ __forceinline__ void tma_load_5d(void* smem_dst, const CUtensorMap* map, unsigned long long* bar,
+                                            int c0, int c1, int c2, int c3, int c4)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];\n"
+        ::"r"(smem_u32(smem_dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
+}
 
 template <typename real, int T_, int BX_, int BY_, int NT_, int PF_>
 struct FusedTraits {
@@ -62,13 +92,18 @@ struct FusedTraits {
     static constexpr int WQ = W / VW;                          // 16-byte groups per row
     static constexpr int NP = RH / 2;                          // row pairs
     static constexpr int G2 = WQ * NP;                         // thread slots (one per row pair x group)
-    static constexpr int PS = W * RH;                          // plane stride in shared memory (elements)
-    static constexpr int GUARD = W;                            // one row before the first and after the last plane
+    static constexpr int A128 = 128 / sizeof(real);            // elements per 128 bytes (TMA destination alignment)
+    static constexpr int HP = ((NP * W + A128 - 1) / A128) * A128;   // half-plane stride: even rows, then odd rows
+    static constexpr int PS = 2 * HP;                          // plane stride in shared memory (elements)
+    static constexpr int GUARD = ((W + A128 - 1) / A128) * A128;     // >= one row before the first / after the last plane
+    static constexpr unsigned HALF_BYTES = (unsigned)(NP * W * sizeof(real));   // bytes one box delivers
     static constexpr int RD = PF + 2;                          // ring depth (planes p+PF .. p+1 in flight, p, p-1)
     static constexpr int XD = 2;                               // exchange planes per stage (written at t, read at t+1)
     static constexpr int NPLANES = 3 * RD + (NS - 1) * XD;
-    static constexpr size_t SMEM_FIXED = ((size_t)NPLANES * PS + 2 * GUARD) * sizeof(real);
+    static constexpr size_t SMEM_FIXED = ((size_t)NPLANES * PS + 2 * GUARD) * sizeof(real) + 128 /*alignment slack*/ + 64 /*mbarriers*/;
     // + (bz + 2H + 2) mask values, added by the launcher
+    static_assert(RD <= 8, "mbarrier block holds 8 barriers");
+    static_assert(H <= PADY && HX <= PADX, "the storage frame must cover the halo");
     static_assert(BX % VW == 0, "tile width must be a multiple of the vector width");
     static_assert(RH % 2 == 0, "rows are owned in pairs");
     static_assert(NT % 32 == 0, "whole warps");
@@ -85,20 +120,23 @@ struct Queue {                       // one z-plane worth of per-thread pipeline
 // GHOSTXY: x or y is a Dirichlet axis, so a tile may hold ghost cells that must stay zero (per-thread mask).
 template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY>
 __global__ void __launch_bounds__(NT, 1)
-fdtd_fused_kernel(const FusedParams P)
+fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
+                  const __grid_constant__ CUtensorMap tmI, const __grid_constant__ CUtensorMap tmV)
 {
     using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
     using V4 = Pack<real>;
     using Q = Queue<real, Tr::NS>;
     constexpr int VW = Tr::VW, NS = Tr::NS, H = Tr::H, HX = Tr::HX, WQ = Tr::WQ, W = Tr::W;
-    constexpr int G2 = Tr::G2, PS = Tr::PS, RD = Tr::RD, XD = Tr::XD;
+    constexpr int G2 = Tr::G2, PS = Tr::PS, HP = Tr::HP, RD = Tr::RD, XD = Tr::XD;
 
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    real* const ringR = reinterpret_cast<real*>(smem_raw) + Tr::GUARD;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    unsigned char* const smem_al = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);   // TMA wants 128-byte aligned boxes
+    real* const ringR = reinterpret_cast<real*>(smem_al) + Tr::GUARD;
     real* const ringI = ringR + RD * PS;
     real* const ringV = ringI + RD * PS;
     real* const exch = ringV + RD * PS;                    // stage s output of iteration t at exch[((s-1)*XD + t%2) * PS]
-    real* const smask = exch + (NS - 1) * XD * PS + Tr::GUARD;  // smask[q] = mask of plane Z0-H-1+q
+    unsigned long long* const full = reinterpret_cast<unsigned long long*>(exch + (NS - 1) * XD * PS + Tr::GUARD);   // full[slot]: plane landed
+    real* const smask = reinterpret_cast<real*>(full + 8); // smask[q] = mask of plane Z0-H-1+q
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int ntiles = P.tiles_x * P.tiles_y;
@@ -119,56 +157,60 @@ fdtd_fused_kernel(const FusedParams P)
     // Threads beyond the last slot repeat the last slot (a halo corner): same loads, same values, no stores.
     const int slot = min(tid, G2 - 1);
     const int rp = slot / WQ, q = slot % WQ;
-    const int soff = (2 * rp) * W + q * VW;          // lo row group inside a plane; hi row at soff + W
+    const int soff = rp * W + q * VW;                // even-row group inside a plane; odd row at soff + HP
     // x neighbours across the warp edge: lane 31 reads the element right of its group, every other lane the
     // element left of lane 0's group (one broadcast address) -- only lanes 0 and 31 use what they read.
     const int soff_lane0 = __shfl_sync(0xffffffffu, soff, 0);
     const int edge_off = (lane == 31) ? VW : (soff_lane0 - 1 - soff);
 
-    unsigned goff[2];    // byte offset of the group inside a plane (wrapped)
-    int ldok[2];         // load from memory (else zero fill: Dirichlet ghost)
+    unsigned goff[2];    // byte offset of the group inside a framed plane
+    int inside[2];       // group lies inside the domain (else: Dirichlet ghost, must stay zero)
     int core[2];         // group belongs to the tile's own cells and lies inside the domain
+    int img_x = 0, img_y[2] = {0, 0};   // byte shifts of the periodic images this thread also stores (0: none)
     {
         const int xg = X0 - HX + q * VW;
-        bool inx = xg >= 0 && xg < P.nx;
-        int xw = xg;
-        if (P.bcx == BC_PERIODIC) { xw = wrap_index(xg, P.nx); inx = true; }
+        const bool inx = P.bcx == BC_PERIODIC || (xg >= 0 && xg < P.nx);
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
             const int r = 2 * rp + j;
             const int yg = Y0 - H + r;
-            bool iny = yg >= 0 && yg < P.ny;
-            int yw = yg;
-            if (P.bcy == BC_PERIODIC) { yw = wrap_index(yg, P.ny); iny = true; }
-            ldok[j] = inx && iny;
-            goff[j] = ldok[j] ? (unsigned)(yw * P.nx + xw) * (unsigned)sizeof(real) : 0u;
+            const bool iny = P.bcy == BC_PERIODIC || (yg >= 0 && yg < P.ny);
+            inside[j] = inx && iny;
+            goff[j] = (unsigned)((yg + PADY) * P.px + xg + PADX) * (unsigned)sizeof(real);
             core[j] = tid < G2 && q * VW >= HX && q * VW < HX + BX && r >= H && r < H + BY &&
                       xg < P.nx && yg < P.ny;   // xg, yg >= 0 is implied for core groups
+            if (core[j] && P.bcy == BC_PERIODIC) {
+                if (yg < PADY) img_y[j] = P.ny * P.px * (int)sizeof(real);
+                else if (yg >= P.ny - PADY) img_y[j] = -P.ny * P.px * (int)sizeof(real);
+            }
+        }
+        if ((core[0] || core[1]) && P.bcx == BC_PERIODIC) {
+            if (xg < PADX) img_x = P.nx * (int)sizeof(real);
+            else if (xg >= P.nx - PADX) img_x = -P.nx * (int)sizeof(real);
         }
     }
+    const bool has_img = (img_x | img_y[0] | img_y[1]) != 0;
 
-    // Byte offsets inside one entry fit 32 bits (the launcher checks cells * sizeof(real) < 4 GiB).
+    // Byte offsets inside one entry fit 32 bits (the launcher checks pcells * sizeof(real) < 4 GiB).
     const unsigned long long ebase = (unsigned long long)b * P.entry_bytes;
-    const char* const bR = static_cast<const char*>(P.Rin) + ebase;
-    const char* const bI = static_cast<const char*>(P.Iin) + ebase;
-    const char* const bV = static_cast<const char*>(P.V) + ebase;
     char* const oR = static_cast<char*>(P.Rout) + ebase;
     char* const oI = static_cast<char*>(P.Iout) + ebase;
-    const unsigned plane_bytes = (unsigned)(P.nx * P.ny) * (unsigned)sizeof(real);
+    const unsigned plane_bytes = (unsigned)(P.px * P.py) * (unsigned)sizeof(real);
 
+    // ---- TMA producer (thread 0): plane pz_next -> ring slot, two half-plane boxes per array ---------
     int pz_next = Z0 - H;                            // next plane to stage (wrapped when z is periodic)
     if (P.bcz == BC_PERIODIC) pz_next = wrap_index(pz_next, P.nz);
-    auto issue_plane = [&](int ring_off) {           // stage the next plane of the march into the ring slot at ring_off
-        const bool zok = (P.bcz == BC_PERIODIC) || (pz_next >= 0 && pz_next < P.nz);
-        const unsigned pb = zok ? (unsigned)pz_next * plane_bytes : 0u;
-        real* dst = ringR + ring_off + soff;
+    const int cx = X0 - HX + PADX, cyp = (Y0 - H + PADY) / 2;   // box origin: x, row pair (Y0-H+PADY is even)
+    auto issue_plane = [&](int ring_off, int slot_idx) {
+        // a Dirichlet ghost plane has an out-of-range z coordinate: the TMA unit fills the box with zeros
+        unsigned long long* bar = full + slot_idx;
+        mbar_expect_tx(bar, 6u * Tr::HALF_BYTES);
+        real* dst = ringR + ring_off;
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
-            const int nbytes = (ldok[j] && zok) ? 16 : 0;      // 0: zero fill (ghost cells)
-            const unsigned o = pb + goff[j];
-            cp_async_16(dst + j * W, bR + o, nbytes);
-            cp_async_16(dst + RD * PS + j * W, bI + o, nbytes);
-            cp_async_16(dst + 2 * RD * PS + j * W, bV + o, nbytes);
+        for (int h = 0; h < 2; ++h) {
+            tma_load_5d(dst + h * HP, &tmR, bar, cx, h, cyp, pz_next, b);
+            tma_load_5d(dst + RD * PS + h * HP, &tmI, bar, cx, h, cyp, pz_next, b);
+            tma_load_5d(dst + 2 * RD * PS + h * HP, &tmV, bar, cx, h, cyp, pz_next, b);
         }
         ++pz_next;
         if (P.bcz == BC_PERIODIC && pz_next == P.nz) pz_next = 0;
@@ -201,24 +243,50 @@ fdtd_fused_kernel(const FusedParams P)
 #pragma unroll
     for (int s = 0; s <= NS; ++s) mq[s] = 0;
 
-    // ---- prologue: PF planes in flight ------------------------------------------------------------
+    // ---- prologue: barriers, PF planes in flight --------------------------------------------------
+    if (tid == 0) {
 #pragma unroll
-    for (int t = 0; t < PF; ++t) { if (t < niter) issue_plane(t * PS); cp_async_commit(); }
+        for (int i = 0; i < RD; ++i) mbar_init(full + i, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+#pragma unroll
+        for (int t = 0; t < PF; ++t) if (t < niter) issue_plane(t * PS, t);
+    }
+    __syncthreads();                                 // barriers initialised before anyone waits on them
     // ring slot offsets (elements) of plane p (cur), p-1 (prev) and of the slot plane p+PF goes to (fill);
     // exchange-plane offsets written this iteration (xw) and read from the previous one (xr)
     auto ring_next = [](int o) { return (o + PS == RD * PS) ? 0 : o + PS; };
     int ro_cur = 0, ro_prev = (RD - 1) * PS, ro_fill = (PF % RD) * PS;
+    int sl_cur = 0, sl_fill = PF % RD;               // the same as slot indices (barrier array)
+    unsigned par = 0;                                // phase parity of full[sl_cur]
     int xw = 0, xr = PS;
 
     unsigned out_pb = (unsigned)(Z0 - H - NS) * plane_bytes;   // byte offset of plane p-NS (wraps harmlessly while p-NS < Z0)
 
+    // the thread's two rows of a finished plane -> global memory, plus their periodic images inside the frame
+    auto store_rows = [&](char* base, unsigned pb, const V4 (&out)[2]) {
+#pragma unroll
+        for (int j = 0; j < 2; ++j)
+            if (core[j]) {
+                char* const dst = base + (size_t)(pb + goff[j]);
+                *reinterpret_cast<V4*>(dst) = out[j];
+                if (has_img) {
+                    if (img_x) *reinterpret_cast<V4*>(dst + img_x) = out[j];
+                    if (img_y[j]) *reinterpret_cast<V4*>(dst + img_y[j]) = out[j];
+                    if (img_x && img_y[j]) *reinterpret_cast<V4*>(dst + img_x + img_y[j]) = out[j];
+                }
+            }
+    };
+
     // One iteration of the march: plane p = Z0-H+t has arrived.  `old`/`mid` hold planes p-s-2 / p-s-1 of
     // every stage s; `nw` receives plane p-s.  (old, mid, nw) rotate by renaming: see the calls below.
     auto body = [&](const int t, Q& old, Q& mid, Q& nw) {
-        cp_async_wait<PF - 1>();
-        __syncthreads();
-        if (t + PF < niter) issue_plane(ro_fill);
-        cp_async_commit();
+        __syncthreads();                             // everyone is done with iteration t-1 (ring slot p-2, exchange planes)
+        if (tid == 0 && t + PF < niter) {
+            asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // generic reads of the slot before the async refill
+            issue_plane(ro_fill, sl_fill);
+        }
+        mbar_wait(full + sl_cur, par);               // plane p has landed
 
         const int p = Z0 - H + t;
 #pragma unroll
@@ -230,9 +298,9 @@ fdtd_fused_kernel(const FusedParams P)
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
             if (NS > 3) dg_oldest[j] = nw.dg[j];     // created three iterations ago: plane p-4
-            nw.f[0][j] = *reinterpret_cast<const V4*>(ringR + ro_cur + soff + j * W);
-            iold[j] = *reinterpret_cast<const V4*>(ringI + ro_prev + soff + j * W);
-            const V4 vraw = *reinterpret_cast<const V4*>(ringV + ro_prev + soff + j * W);
+            nw.f[0][j] = *reinterpret_cast<const V4*>(ringR + ro_cur + soff + j * HP);
+            iold[j] = *reinterpret_cast<const V4*>(ringI + ro_prev + soff + j * HP);
+            const V4 vraw = *reinterpret_cast<const V4*>(ringV + ro_prev + soff + j * HP);
 #pragma unroll
             for (int e = 0; e < VW; ++e) nw.dg[j].e[e] = fma(cv, vraw.e[e], c6);
         }
@@ -241,11 +309,11 @@ fdtd_fused_kernel(const FusedParams P)
         for (int s = 1; s <= NS; ++s) {
             // plane holding the centre values of this stage (written during the previous iteration)
             const real* cplane = ((s == 1) ? (ringR + ro_prev) : (exch + (s >= 2 ? s - 2 : 0) * XD * PS + xr)) + soff;
-            const V4 ym = *reinterpret_cast<const V4*>(cplane - W);          // row 2rp-1
-            const V4 yp = *reinterpret_cast<const V4*>(cplane + 2 * W);      // row 2rp+2
+            const V4 ym = *reinterpret_cast<const V4*>(cplane + HP - W);     // row 2rp-1: odd row of pair rp-1
+            const V4 yp = *reinterpret_cast<const V4*>(cplane + W);          // row 2rp+2: even row of pair rp+1
             real edge[2];
             edge[0] = cplane[edge_off];
-            edge[1] = cplane[W + edge_off];
+            edge[1] = cplane[HP + edge_off];
             V4 out[2];
 #pragma unroll
             for (int j = 0; j < 2; ++j) {
@@ -260,7 +328,7 @@ fdtd_fused_kernel(const FusedParams P)
                 const real xp_s = __shfl_down_sync(0xffffffffu, ctr.e[0], 1);
                 const real xm = (lane == 0) ? edge[j] : xm_s;
                 const real xp = (lane == 31) ? edge[j] : xp_s;
-                const real m = (GHOSTXY && !ldok[j]) ? (real)0 : mq[s];
+                const real m = (GHOSTXY && !inside[j]) ? (real)0 : mq[s];
 #pragma unroll
                 for (int e = 0; e < VW; ++e) {
                     const real left = (e == 0) ? xm : ctr.e[e - 1];
@@ -276,28 +344,22 @@ fdtd_fused_kernel(const FusedParams P)
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
                     nw.f[s][j] = out[j];
-                    *reinterpret_cast<V4*>(exch + (s - 1) * XD * PS + xw + soff + j * W) = out[j];
+                    *reinterpret_cast<V4*>(exch + (s - 1) * XD * PS + xw + soff + j * HP) = out[j];
                 }
             }
             if (s == NS - 1) {                       // I^{n+T-1/2} at plane p-NS+1
                 const int pz = p - (NS - 1);
-                if (pz >= Z0 && pz < Z0 + bzc) {
-#pragma unroll
-                    for (int j = 0; j < 2; ++j)
-                        if (core[j]) *reinterpret_cast<V4*>(oI + (size_t)(out_pb + plane_bytes + goff[j])) = out[j];
-                }
+                if (pz >= Z0 && pz < Z0 + bzc) store_rows(oI, out_pb + plane_bytes, out);
             }
             if (s == NS) {                           // R^{n+T} at plane p-NS
                 const int pz = p - NS;
-                if (pz >= Z0 && pz < Z0 + bzc) {
-#pragma unroll
-                    for (int j = 0; j < 2; ++j)
-                        if (core[j]) *reinterpret_cast<V4*>(oR + (size_t)(out_pb + goff[j])) = out[j];
-                }
+                if (pz >= Z0 && pz < Z0 + bzc) store_rows(oR, out_pb, out);
             }
         }
         out_pb += plane_bytes;
         ro_prev = ro_cur; ro_cur = ring_next(ro_cur); ro_fill = ring_next(ro_fill);
+        if (++sl_cur == RD) { sl_cur = 0; par ^= 1u; }
+        if (++sl_fill == RD) sl_fill = 0;
         xr = xw; xw = PS - xw;
     };
 
@@ -309,7 +371,6 @@ fdtd_fused_kernel(const FusedParams P)
         if (t + 2 >= niter) break;
         body(t + 2, qc, qa, qb);
     }
-    cp_async_wait<0>();
 }
 
 }  // namespace tdse

@@ -36,8 +36,9 @@ def test_library_exports_every_declared_symbol(lib):
 def test_workspace_bytes_is_pure_host_arithmetic(lib):
     n3 = lib.tdse_workspace_bytes(64, 64, 64, 1, pkg.TDSE_F64, 0)
     n5 = lib.tdse_workspace_bytes(64, 64, 64, 1, pkg.TDSE_F64, 1)
-    assert n3 == 3 * 64 ** 3 * 8 and n5 == 5 * 64 ** 3 * 8
-    assert lib.tdse_workspace_bytes(5, 3, 7, 2, pkg.TDSE_F32, 0) == 3 * 1024   # 840 B rounded up to 256-B multiples
+    # device storage frames every xy plane with 4 columns / 4 rows on each side (include/tdse.h, tdse_workspace_bytes)
+    assert n3 == 3 * 72 * 72 * 64 * 8 and n5 == 5 * 72 * 72 * 64 * 8
+    assert lib.tdse_workspace_bytes(5, 3, 7, 2, pkg.TDSE_F32, 0) == 3 * 8192   # 13*11*7*2*4 = 8008 B rounded up to 256-B multiples
     assert lib.tdse_workspace_bytes(0, 3, 7, 2, pkg.TDSE_F32, 0) == 0
     assert lib.tdse_workspace_bytes(4, 4, 4, 1, 7, 0) == 0
 

@@ -68,11 +68,29 @@ SHAPES = [(72, 40, 37), (64, 64, 16), (8, 6, 5), (136, 70, 21), (4, 3, 2)]
 VARIANTS = [(TWOPASS, 1), (FUSED, 1), (FUSED, 2)]
 
 
+def fused_eligible(nx, ny, dtype):
+    """include/tdse.h, tdse_set_option("kernel"): 16-byte rows, even ny, domain at least as wide as two frames."""
+    return nx % (4 if dtype == "f32" else 2) == 0 and ny % 2 == 0 and nx >= 8 and ny >= 8
+
+
 @pytest.mark.parametrize("kernel,tblock", VARIANTS)
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("shape,bc", list(zip(SHAPES, BCS)) + [((40, 24, 30), BCS[2]), ((40, 24, 30), BCS[1])])
+@pytest.mark.parametrize("shape,bc", list(zip(SHAPES, BCS)) + [((40, 24, 30), BCS[2]), ((40, 24, 30), BCS[1]),
+                                                               ((8, 8, 5), BCS[2]), ((8, 8, 3), BCS[4])])
 def test_recurrence_matches_oracle_on_random_states(kernel, tblock, dtype, shape, bc):
     nx, ny, nz = shape
+    if kernel == FUSED and not fused_eligible(nx, ny, dtype):
+        # forcing the fused kernel on a shape it does not take must fail loudly, not fall back
+        t = make_ctx(nx, ny, nz, 1, 0.25, 0.004, dtype)
+        t.set_option("kernel", FUSED)
+        t.set_potential_grid(0, np.zeros((nz, ny, nx), dtype=t.np_dtype))
+        t.set_state(0, np.ones((nz, ny, nx), dtype=t.np_dtype), np.ones((nz, ny, nx), dtype=t.np_dtype))
+        from paper_2401_07416_b200 import TdseError, TDSE_EINVAL
+        with pytest.raises(TdseError) as ei:
+            t.step(1)
+        assert ei.value.code == TDSE_EINVAL
+        t.close()
+        return
     dx, dt, steps, batch = 0.25, 0.004, 23, 2
     absorb = min(4, nz // 3)
     t = make_ctx(nx, ny, nz, batch, dx, dt, dtype)
