@@ -10,54 +10,106 @@ struct AtomRec { double x, y, z, Z, soft2, screen; };   // same layout as tdse_a
 
 // ---------------------------------------------------------------------------------------------
 // S0 potential build (BASELINE.json north_star (1)): V = clamp(sum_a -Z_a exp(-r_a/lambda_a)/sqrt(r_a^2+s_a^2)).
-// One thread per cell, x fastest; atoms staged through shared memory in chunks; double accumulate in
-// list order; one rounding to `real`.  Nearest image on periodic axes.
+// Bound by the fp64 pipe (exp, two inverse square roots per cell-atom pair), so the work per pair is cut
+// down: a thread owns kPotCells consecutive cells along x and shares the y/z part of the distance among
+// them; atoms are staged through shared memory in chunks with 1/lambda precomputed; exp(-r/lambda) is an
+// inline range reduction + degree-13 polynomial (|error| < 1 ulp for arguments <= 0), r = r2 * rsqrt(r2).
+// Double accumulate in list order, one rounding to `real`.  Nearest image on periodic axes.
 // ---------------------------------------------------------------------------------------------
 constexpr int kAtomChunk = 128;
+constexpr int kPotCells = 4;
+
+struct AtomStaged { double x, y, z, Z, soft2, inv_screen; };   // inv_screen = 0: unscreened
+
+// exp(x) for x <= 0 (flushes to 0 below -708: smaller than any double the sum can register)
+__device__ __forceinline__ double exp_nonpositive(double x)
+{
+    if (x < -708.0) return 0.0;
+    const double magic = 6755399441055744.0;                       // 1.5 * 2^52: round to nearest integer
+    double t = fma(x, 1.4426950408889634074, magic);
+    const int k = __double2loint(t);
+    t -= magic;
+    double r = fma(t, -6.93147180369123816490e-01, x);
+    r = fma(t, -1.90821492927058770002e-10, r);                    // |r| <= ln2 / 2
+    double p = 1.0 / 6227020800.0;                                 // Taylor to r^13: remainder < 5e-18
+    p = fma(p, r, 1.0 / 479001600.0);
+    p = fma(p, r, 1.0 / 39916800.0);
+    p = fma(p, r, 1.0 / 3628800.0);
+    p = fma(p, r, 1.0 / 362880.0);
+    p = fma(p, r, 1.0 / 40320.0);
+    p = fma(p, r, 1.0 / 5040.0);
+    p = fma(p, r, 1.0 / 720.0);
+    p = fma(p, r, 1.0 / 120.0);
+    p = fma(p, r, 1.0 / 24.0);
+    p = fma(p, r, 1.0 / 6.0);
+    p = fma(p, r, 0.5);
+    p = fma(p, r, 1.0);
+    p = fma(p, r, 1.0);
+    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));   // p * 2^k, k >= -1022
+}
 
 template <typename real>
 __global__ void __launch_bounds__(256)
 potential_build_kernel(Grid g, double dx, const AtomRec* __restrict__ atoms, int natoms,
                        double vmin, double vmax, double rcut, real* __restrict__ V /* entry base */)
 {
-    __shared__ AtomRec s_atoms[kAtomChunk];
-    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = cell < g.cells;
-    int i = 0, j = 0, k = 0;
+    __shared__ AtomStaged s_atoms[kAtomChunk];
+    const int nxq = (g.nx + kPotCells - 1) / kPotCells;
+    const long long slot = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = slot < (long long)nxq * g.ny * g.nz;
+    int i0 = 0, j = 0, k = 0;
     if (live) {
-        i = (int)(cell % g.nx);
-        const long long t = cell / g.nx;
+        i0 = (int)(slot % nxq) * kPotCells;
+        const long long t = slot / nxq;
         j = (int)(t % g.ny);
         k = (int)(t / g.ny);
     }
-    const double x = i * dx, y = j * dx, z = k * dx;
+    const double y = j * dx, z = k * dx;
     const double Lx = g.nx * dx, Ly = g.ny * dx, Lz = g.nz * dx;
-    double sum = 0.0;
+    const double iLx = 1.0 / Lx, iLy = 1.0 / Ly, iLz = 1.0 / Lz;
+    const bool perx = g.bcx == BC_PERIODIC, pery = g.bcy == BC_PERIODIC, perz = g.bcz == BC_PERIODIC;
+    const double rc2 = rcut * rcut;
+    double sum[kPotCells];
+#pragma unroll
+    for (int e = 0; e < kPotCells; ++e) sum[e] = 0.0;
     for (int a0 = 0; a0 < natoms; a0 += kAtomChunk) {
         const int na = min(kAtomChunk, natoms - a0);
         __syncthreads();
-        for (int q = threadIdx.x; q < na * 6; q += blockDim.x)
-            reinterpret_cast<double*>(s_atoms)[q] = reinterpret_cast<const double*>(atoms + a0)[q];
+        for (int q = threadIdx.x; q < na; q += blockDim.x) {
+            const AtomRec A = atoms[a0 + q];
+            AtomStaged S;
+            S.x = A.x; S.y = A.y; S.z = A.z; S.Z = A.Z; S.soft2 = A.soft2;
+            S.inv_screen = (A.screen > 0.0 && isfinite(A.screen)) ? 1.0 / A.screen : 0.0;
+            s_atoms[q] = S;
+        }
         __syncthreads();
-        if (live) {
-            for (int a = 0; a < na; ++a) {
-                const AtomRec A = s_atoms[a];
-                double ddx = x - A.x, ddy = y - A.y, ddz = z - A.z;
-                if (g.bcx == BC_PERIODIC) ddx = ddx - Lx * round(ddx / Lx);
-                if (g.bcy == BC_PERIODIC) ddy = ddy - Ly * round(ddy / Ly);
-                if (g.bcz == BC_PERIODIC) ddz = ddz - Lz * round(ddz / Lz);
-                const double r2 = ddx * ddx + ddy * ddy + ddz * ddz;
-                const double r = sqrt(r2);
-                if (rcut > 0.0 && r > rcut) continue;
-                double screen = 1.0;
-                if (A.screen > 0.0 && isfinite(A.screen)) screen = exp(-r / A.screen);
-                sum += -A.Z * screen / sqrt(r2 + A.soft2);
+        if (!live) continue;
+        for (int a = 0; a < na; ++a) {
+            const AtomStaged A = s_atoms[a];
+            double ddy = y - A.y, ddz = z - A.z;
+            if (pery) ddy = fma(-Ly, rint(ddy * iLy), ddy);
+            if (perz) ddz = fma(-Lz, rint(ddz * iLz), ddz);
+            const double yz2 = fma(ddy, ddy, ddz * ddz);
+#pragma unroll
+            for (int e = 0; e < kPotCells; ++e) {
+                double ddx = (i0 + e) * dx - A.x;
+                if (perx) ddx = fma(-Lx, rint(ddx * iLx), ddx);
+                const double r2 = fma(ddx, ddx, yz2);
+                double r = r2 > 0.0 ? r2 * rsqrt(r2) : 0.0;
+                if (rcut > 0.0) {
+                    // the cutoff is defined on r = sqrt(r2) (correctly rounded): decide on r2 unless it is a tie
+                    if (fabs(r2 - rc2) <= 1e-12 * rc2) r = sqrt(r2);
+                    if (r > rcut) continue;
+                }
+                const double screen = A.inv_screen > 0.0 ? exp_nonpositive(-r * A.inv_screen) : 1.0;
+                sum[e] = fma(-A.Z * screen, rsqrt(r2 + A.soft2), sum[e]);
             }
         }
     }
     if (live) {
-        sum = fmin(fmax(sum, vmin), vmax);
-        store_with_images(V, g, i, j, k, (real)sum);
+#pragma unroll
+        for (int e = 0; e < kPotCells; ++e)
+            if (i0 + e < g.nx) store_with_images(V, g, i0 + e, j, k, (real)fmin(fmax(sum[e], vmin), vmax));
     }
 }
 
