@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--tblock", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--agreement", action="store_true",
+                    help="cfg4: also run 384^3 in f32 and f64 (batch 1, full step count) and report the rel-L2 of the detector images")
     return ap.parse_args()
 
 
@@ -183,6 +185,20 @@ def cpu_baseline(w):
     t0 = time.perf_counter(); o.step(n); dt = time.perf_counter() - t0
     return {"value": w.cells * n / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": "entry 0 of %s, %d of %d FDTD steps (%.1f s)" % (w.name, n, w.steps, dt)}
+
+
+def fp32_vs_fp64_agreement(device):
+    """BASELINE.json configs[4]: fp32-vs-fp64 agreement on the detector intensity, same 384^3 grid for both dtypes."""
+    from paper_2401_07416_b200 import Tdse
+    imgs = {}
+    for dt_ in ("f32", "f64"):
+        w = make_config(4, dtype=dt_, n=(384, 384, 384), batch=1)
+        t = Tdse.from_workload(w, device=device)
+        t.step(w.steps)
+        imgs[dt_], _ = t.detector_read(0)
+        t.close()
+    d = float(np.linalg.norm(imgs["f32"] - imgs["f64"]) / np.linalg.norm(imgs["f64"]))
+    return {"grid": [384, 384, 384], "fdtd_steps": int(w.steps), "detector_rel_l2_f32_vs_f64": d}
 
 
 def main():
@@ -345,6 +361,9 @@ def main():
             "trajectories_per_hour": 3600.0 * w.batch * world * a.steps / (total_ms * 1e-3),
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
         }
+        if a.agreement and idx == 4:
+            t.close()
+            line["fp32_vs_fp64"] = fp32_vs_fp64_agreement("cuda:%d" % local_rank)
         print(json.dumps(line), flush=True)
     t.close()
     if world > 1:
