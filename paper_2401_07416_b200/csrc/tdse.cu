@@ -227,8 +227,8 @@ bool entry_range(const tdse_ctx* c, int b, int* b0, int* b1)
 }
 
 // ---------------------------------------------------------------------------------------------
-// TMA descriptors for the fused kernel: the 5-d view (x, row parity, row pair, z, entry) of one framed
-// array, box = one half-plane of a tile (W x 1 x NP x 1 x 1).  cuTensorMapEncodeTiled is taken from the
+// TMA descriptors for the fused kernel: the 5-d view (x, row pair, row parity, z, entry) of one framed
+// array, box = one tile plane (W x NP x 2 x 1 x 1), which lands as [parity][pair][x].  cuTensorMapEncodeTiled is taken from the
 // driver through the runtime (no link against libcuda).
 // ---------------------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -260,9 +260,9 @@ int get_tensor_maps(tdse_ctx* c, int W, int NP, const CUtensorMap** out)
         std::vector<CUtensorMap> maps(5);
         void* arrs[5] = {c->R[0], c->I[0], c->V, c->R[1], c->I[1]};
         const cuuint64_t w = c->w, px = (cuuint64_t)c->g.px, py = (cuuint64_t)c->g.py;
-        const cuuint64_t dims[5] = {px, 2, py / 2, (cuuint64_t)c->g.nz, (cuuint64_t)c->g.batch};
-        const cuuint64_t strides[4] = {px * w, 2 * px * w, px * py * w, px * py * (cuuint64_t)c->g.nz * w};
-        const cuuint32_t box[5] = {(cuuint32_t)W, 1, (cuuint32_t)NP, 1, 1};
+        const cuuint64_t dims[5] = {px, py / 2, 2, (cuuint64_t)c->g.nz, (cuuint64_t)c->g.batch};
+        const cuuint64_t strides[4] = {2 * px * w, px * w, px * py * w, px * py * (cuuint64_t)c->g.nz * w};
+        const cuuint32_t box[5] = {(cuuint32_t)W, (cuuint32_t)NP, 2, 1, 1};
         const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
         for (int a = 0; a < 5; ++a) {
             const CUresult r = enc(&maps[a], c->dtype == TDSE_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64,
@@ -279,12 +279,12 @@ int get_tensor_maps(tdse_ctx* c, int W, int NP, const CUtensorMap** out)
 // ---------------------------------------------------------------------------------------------
 // fused launch table
 // ---------------------------------------------------------------------------------------------
-template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY>
-int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm)
+template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY, int MINB = 1>
+int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
 {
     using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
-    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF, GHOSTXY>;
-    constexpr size_t kMaxSmem = 227 * 1024;
+    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF, GHOSTXY, MINB>;
+    constexpr size_t kMaxSmem = MINB == 1 ? 227 * 1024 : (228 * 1024) / MINB - 1024;   // per CTA (1 KB reserved each)
     static_assert(Tr::SMEM_FIXED + 64 * sizeof(real) <= kMaxSmem, "fused tile does not fit in shared memory");
     static bool attr_set = false;
     if (!attr_set) {

@@ -14,8 +14,8 @@
 //     elected thread, mbarrier completion, PF planes ahead).  Device storage carries a frame of periodic
 //     images / Dirichlet zeros around every xy plane (tdse_common.cuh), so a box never wraps in x or y;
 //     out-of-range z planes (Dirichlet ghosts) are zero-filled by the TMA unit, periodic z wraps the plane
-//     index.  The 5-d tensor view (x, row parity, row pair, z, entry) splits even and odd rows into two
-//     half-planes so that every 16-byte shared-memory access of a warp is contiguous (no bank conflicts);
+//     index.  The 5-d tensor view (x, row pair, row parity, z, entry) makes one box land as two
+//     half-planes (even rows, odd rows) so that every 16-byte shared-memory access of a warp is contiguous;
 //   * a thread owns a 2-row x 16-byte patch of the tile (rows 2rp, 2rp+1).  Per stage it keeps the previous
 //     two z-planes of its cells in registers (register-rotated z neighbours: the march is unrolled by 3 so
 //     the rotation costs no moves); the y neighbour between its two rows is a register, the outer two y
@@ -71,13 +71,25 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned pari
         "DONE_%=:\n"
         "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-// one half-plane box (W x 1 x NP x 1 x 1) of the 5-d view (x, row parity, row pair, z, entry)
+// one box (W x NP x 2 x 1 x 1) of the 5-d view (x, row pair, row parity, z, entry): lands as [parity][pair][x]
 __device__ __forceinline__ void tma_load_5d(void* smem_dst, const CUtensorMap* map, unsigned long long* bar,
                                             int c0, int c1, int c2, int c3, int c4)
 {
     asm volatile(
         "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];\n"
         ::"r"(smem_u32(smem_dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
+}
+
+// 16-byte global store under a predicate (no branch)
+__device__ __forceinline__ void st_global_pred(void* p, const Pack<float>& v, int pred)
+{
+    asm volatile("{\n.reg .pred q;\nsetp.ne.s32 q, %5, 0;\n@q st.global.v4.f32 [%0], {%1, %2, %3, %4};\n}\n"
+                 ::"l"(p), "f"(v.e[0]), "f"(v.e[1]), "f"(v.e[2]), "f"(v.e[3]), "r"(pred) : "memory");
+}
+__device__ __forceinline__ void st_global_pred(void* p, const Pack<double>& v, int pred)
+{
+    asm volatile("{\n.reg .pred q;\nsetp.ne.s32 q, %3, 0;\n@q st.global.v2.f64 [%0], {%1, %2};\n}\n"
+                 ::"l"(p), "d"(v.e[0]), "d"(v.e[1]), "r"(pred) : "memory");
 }
 
 template <typename real, int T_, int BX_, int BY_, int NT_, int PF_>
@@ -93,10 +105,11 @@ struct FusedTraits {
     static constexpr int NP = RH / 2;                          // row pairs
     static constexpr int G2 = WQ * NP;                         // thread slots (one per row pair x group)
     static constexpr int A128 = 128 / sizeof(real);            // elements per 128 bytes (TMA destination alignment)
-    static constexpr int HP = ((NP * W + A128 - 1) / A128) * A128;   // half-plane stride: even rows, then odd rows
+    static constexpr int HP = NP * W;                          // half-plane stride: even rows, then odd rows (one dense TMA box)
     static constexpr int PS = 2 * HP;                          // plane stride in shared memory (elements)
     static constexpr int GUARD = ((W + A128 - 1) / A128) * A128;     // >= one row before the first / after the last plane
-    static constexpr unsigned HALF_BYTES = (unsigned)(NP * W * sizeof(real));   // bytes one box delivers
+    static constexpr unsigned BOX_BYTES = (unsigned)(PS * sizeof(real));        // bytes one box (W x NP x 2) delivers
+    static_assert((PS * sizeof(real)) % 128 == 0, "ring slots must stay 128-byte aligned for TMA");
     static constexpr int RD = PF + 2;                          // ring depth (planes p+PF .. p+1 in flight, p, p-1)
     static constexpr int XD = 2;                               // exchange planes per stage (written at t, read at t+1)
     static constexpr int NPLANES = 3 * RD + (NS - 1) * XD;
@@ -118,8 +131,9 @@ struct Queue {                       // one z-plane worth of per-thread pipeline
 };
 
 // GHOSTXY: x or y is a Dirichlet axis, so a tile may hold ghost cells that must stay zero (per-thread mask).
-template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY>
-__global__ void __launch_bounds__(NT, 1)
+// MINB: CTAs that must fit on one SM (small tiles run several independent CTAs per SM).
+template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY, int MINB = 1>
+__global__ void __launch_bounds__(NT, MINB)
 fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
                   const __grid_constant__ CUtensorMap tmI, const __grid_constant__ CUtensorMap tmV)
 {
@@ -189,7 +203,8 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
             else if (xg >= P.nx - PADX) img_x = -P.nx * (int)sizeof(real);
         }
     }
-    const bool has_img = (img_x | img_y[0] | img_y[1]) != 0;
+    const bool warp_img_x = __any_sync(0xffffffffu, img_x != 0);                 // warp-uniform: no divergence
+    const bool warp_img_y = __any_sync(0xffffffffu, (img_y[0] | img_y[1]) != 0);
 
     // Byte offsets inside one entry fit 32 bits (the launcher checks pcells * sizeof(real) < 4 GiB).
     const unsigned long long ebase = (unsigned long long)b * P.entry_bytes;
@@ -204,14 +219,11 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
     auto issue_plane = [&](int ring_off, int slot_idx) {
         // a Dirichlet ghost plane has an out-of-range z coordinate: the TMA unit fills the box with zeros
         unsigned long long* bar = full + slot_idx;
-        mbar_expect_tx(bar, 6u * Tr::HALF_BYTES);
+        mbar_expect_tx(bar, 3u * Tr::BOX_BYTES);
         real* dst = ringR + ring_off;
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            tma_load_5d(dst + h * HP, &tmR, bar, cx, h, cyp, pz_next, b);
-            tma_load_5d(dst + RD * PS + h * HP, &tmI, bar, cx, h, cyp, pz_next, b);
-            tma_load_5d(dst + 2 * RD * PS + h * HP, &tmV, bar, cx, h, cyp, pz_next, b);
-        }
+        tma_load_5d(dst, &tmR, bar, cx, cyp, 0, pz_next, b);
+        tma_load_5d(dst + RD * PS, &tmI, bar, cx, cyp, 0, pz_next, b);
+        tma_load_5d(dst + 2 * RD * PS, &tmV, bar, cx, cyp, 0, pz_next, b);
         ++pz_next;
         if (P.bcz == BC_PERIODIC && pz_next == P.nz) pz_next = 0;
     };
@@ -265,28 +277,31 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
 
     // the thread's two rows of a finished plane -> global memory, plus their periodic images inside the frame
     auto store_rows = [&](char* base, unsigned pb, const V4 (&out)[2]) {
-#pragma unroll
-        for (int j = 0; j < 2; ++j)
-            if (core[j]) {
-                char* const dst = base + (size_t)(pb + goff[j]);
-                *reinterpret_cast<V4*>(dst) = out[j];
-                if (has_img) {
-                    if (img_x) *reinterpret_cast<V4*>(dst + img_x) = out[j];
-                    if (img_y[j]) *reinterpret_cast<V4*>(dst + img_y[j]) = out[j];
-                    if (img_x && img_y[j]) *reinterpret_cast<V4*>(dst + img_x + img_y[j]) = out[j];
-                }
-            }
+        // predicated 16-byte stores, no divergent branches (a branch region per row and image cost more than the
+        // stores themselves: profiles/README.md); only warps that hold a y-face row enter the y-image part
+        char* const d0 = base + (size_t)(pb + goff[0]);
+        char* const d1 = base + (size_t)(pb + goff[1]);
+        st_global_pred(d0, out[0], core[0]);
+        st_global_pred(d1, out[1], core[1]);
+        if (warp_img_x) {
+            st_global_pred(d0 + img_x, out[0], core[0] && img_x);
+            st_global_pred(d1 + img_x, out[1], core[1] && img_x);
+        }
+        if (warp_img_y) {
+            st_global_pred(d0 + img_y[0], out[0], img_y[0]);
+            st_global_pred(d1 + img_y[1], out[1], img_y[1]);
+            st_global_pred(d0 + img_y[0] + img_x, out[0], img_y[0] && img_x);
+            st_global_pred(d1 + img_y[1] + img_x, out[1], img_y[1] && img_x);
+        }
     };
 
     // One iteration of the march: plane p = Z0-H+t has arrived.  `old`/`mid` hold planes p-s-2 / p-s-1 of
     // every stage s; `nw` receives plane p-s.  (old, mid, nw) rotate by renaming: see the calls below.
     auto body = [&](const int t, Q& old, Q& mid, Q& nw) {
+        mbar_wait(full + sl_cur, par);               // plane p has landed (issued PF iterations ago)
         __syncthreads();                             // everyone is done with iteration t-1 (ring slot p-2, exchange planes)
-        if (tid == 0 && t + PF < niter) {
-            asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");   // generic reads of the slot before the async refill
-            issue_plane(ro_fill, sl_fill);
-        }
-        mbar_wait(full + sl_cur, par);               // plane p has landed
+        // refill the slot of plane p-2: its last readers passed the barrier above (reads ordered before the async write)
+        if (tid == 0 && t + PF < niter) issue_plane(ro_fill, sl_fill);
 
         const int p = Z0 - H + t;
 #pragma unroll
