@@ -6,7 +6,9 @@ The arithmetic lives in plain C (tdse_oracle.c, tdse_oracle_step.inc); this modu
 that file with gcc and marshals numpy arrays through ctypes.
 """
 from .driver import (build, lib, OracleRun, potential, mask, wavepacket, stagger,
-                     coefficients, max_threads, set_threads, paper_time_step, paper_wavelength)
+                     coefficients, max_threads, set_threads, paper_time_step, paper_wavelength,
+                     dissimilarity)
 
 __all__ = ["build", "lib", "OracleRun", "potential", "mask", "wavepacket", "stagger",
-           "coefficients", "max_threads", "set_threads", "paper_time_step", "paper_wavelength"]
+           "coefficients", "max_threads", "set_threads", "paper_time_step", "paper_wavelength",
+           "dissimilarity"]

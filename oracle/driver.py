@@ -57,6 +57,11 @@ def lib():
                 g = getattr(L, "oracle_norm_" + sfx)
                 g.restype = None
                 g.argtypes = [C.c_int] * 6 + [C.c_double] * 5 + [rp, rp, rp, rp, dp, dp]
+                h = getattr(L, "oracle_plane_density_" + sfx)
+                h.restype = None
+                h.argtypes = [C.c_int] * 3 + [rp, rp, dp]
+            L.oracle_dissimilarity.restype = C.c_double
+            L.oracle_dissimilarity.argtypes = [dp, dp, C.c_int, C.c_double, C.c_int, C.c_int]
             _LIB = L
     return _LIB
 
@@ -123,6 +128,15 @@ def stagger(bc, coef, V, R0, J0) -> np.ndarray:
     return out
 
 
+def dissimilarity(frames_k, frames_j, dA: float, s0: int, s1: int) -> float:
+    """eq (16), over the frames s0..s1 (inclusive) of two [nframes][ny][nx] trajectories."""
+    a = np.ascontiguousarray(frames_k, dtype=np.float64)
+    b = np.ascontiguousarray(frames_j, dtype=np.float64)
+    assert a.shape == b.shape and 0 <= s0 <= s1 < a.shape[0]
+    npix = int(np.prod(a.shape[1:]))
+    return float(lib().oracle_dissimilarity(_p(a, C.c_double), _p(b, C.c_double), npix, float(dA), int(s0), int(s1)))
+
+
 class OracleRun:
     """One batch entry of the hot path, step by step.
 
@@ -152,6 +166,8 @@ class OracleRun:
         self.D = np.zeros((self.ny, self.nx), dtype=np.float64)
         self.trace = []
         self.counter = C.c_longlong(0)
+        self.keep_frames, self.include_t0 = False, True
+        self.frames = []              # frame mode: rho at s = 0 (optional), h, 2h, ...
 
     # -- rounding of inputs to the run's storage dtype --------------------------------
     def _round(self, a: np.ndarray) -> np.ndarray:
@@ -196,9 +212,37 @@ class OracleRun:
         self.counter = C.c_longlong(0)
         return self
 
+    def set_frames(self, keep: bool = True, include_t0: bool = True):
+        """Frame mode: keep every sampled detector frame (the paper's trajectory rho = {rho(0), rho(h dt), ...})."""
+        self.keep_frames, self.include_t0 = bool(keep), bool(include_t0)
+        self.frames = []
+        return self
+
+    def plane_density(self) -> np.ndarray:
+        ct = C.c_double if self.dtype == "f64" else C.c_float
+        rho = np.empty((self.ny, self.nx), dtype=np.float64)
+        getattr(lib(), "oracle_plane_density_" + self.dtype)(self.nx, self.ny, self.k_det, _p(self.R, ct), _p(self.I, ct),
+                                                             _p(rho, C.c_double))
+        return rho
+
     # -- the recurrence -------------------------------------------------------------
     def step(self, n: int):
         assert self.V is not None and self.R is not None
+        if self.keep_frames and self.every > 0:
+            # advance from one sampling step to the next so that a frame can be taken from the state in memory
+            if self.counter.value == 0 and self.include_t0 and not self.frames:
+                self.frames.append(self.plane_density())
+            left = int(n)
+            while left > 0:
+                m = min(left, self.every - int(self.counter.value % self.every))
+                self._advance(m)
+                left -= m
+                if self.counter.value % self.every == 0:
+                    self.frames.append(self.plane_density())
+            return self
+        return self._advance(n)
+
+    def _advance(self, n: int):
         ct = C.c_double if self.dtype == "f64" else C.c_float
         f = getattr(lib(), "oracle_step_" + self.dtype)
         cap = n // self.every + 2 if self.every > 0 else 1

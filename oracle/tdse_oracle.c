@@ -18,6 +18,8 @@
  *   oracle_stagger     I^{-1/2} = Im psi0 + (1/2) A Re psi0   (reading 4).
  *   oracle_step_*      eqs (8), (9), (13), (14), (15): see tdse_oracle_step.inc.
  *   oracle_norm_*      PAPER.md:87 density and the conserved Visscher form.
+ *   oracle_plane_density_*  one detector frame rho(i,j) = R^2 + I^2 on plane k_det (eq (15)).
+ *   oracle_dissimilarity    eq (16), between two frame trajectories (reading 23).
  *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): dense-eigh closed form on tiny grids, FFT
  * closed form, exact expm propagation + second-order convergence, conservation of q_visscher,
@@ -173,3 +175,23 @@ void oracle_stagger(int nx, int ny, int nz, int bcx, int bcy, int bcz,
 #include "tdse_oracle_step.inc"
 #undef REAL
 #undef NAME
+
+/* Dissimilarity of two detector-plane trajectories, eq (16) PAPER.md:219-221:
+ *   d_kj = 1/(t1 - t0) * int_{t0}^{t1} ( int_D ( rho_k(r,t) - rho_j(r,t) )^2 dr )^{1/2} dt
+ * rho_k, rho_j: [nframes][npix] frames of |psi|^2 on the detector plane at equally spaced times.
+ * Reading: int_D dr -> dA * sum over pixels; the time average over the window
+ * [t0, t1] -> the arithmetic mean over the frames s0 .. s1 (inclusive) that fall in it.
+ * Serial sums in double, pixels in row-major order, frames in increasing order. */
+double oracle_dissimilarity(const double* rho_k, const double* rho_j, int npix, double dA, int s0, int s1)
+{
+    double acc = 0.0;
+    for (int s = s0; s <= s1; ++s) {
+        double inner = 0.0;
+        for (int p = 0; p < npix; ++p) {
+            const double d = rho_k[(size_t)s * npix + p] - rho_j[(size_t)s * npix + p];
+            inner += d * d;
+        }
+        acc += sqrt(dA * inner);
+    }
+    return acc / (double)(s1 - s0 + 1);
+}

@@ -419,3 +419,76 @@ def test_paper_time_step_and_coefficients():
     lam = oracle.paper_wavelength(60.0 * si["eV_J"], si["electron_mass_kg"], si["hbar_Js"])
     assert abs(lam / 1e-10 - si["de_broglie_angstrom_sqrt_eV"] / math.sqrt(60.0)) < 2e-5
     assert 140 * 140 * (420 + g["cap_planes"]["value"]) == g["mesh_points_small"]["value"]
+
+
+# ---------------------------------------------------------------------------------------
+# frame-mode detector and trajectory dissimilarity (eq 16)
+# ---------------------------------------------------------------------------------------
+def test_frames_against_fft_closed_form_and_accumulated_image():
+    """Frames are (R^s)^2 + (I^{s-1/2})^2 on the plane at s = 0, h, 2h, ...: pinned with the discrete-exact
+    Fourier solution of the free periodic recurrence (independent of the oracle), and with the identities
+    sum_{s>=1} frame_s = accumulated image, trace_s = dx^2 sum(frame_s)."""
+    nx, ny, nz = 16, 12, 20
+    dx, dt, h, k_det = 0.25, 0.008, 7, 5
+    R0, I0 = random_state(11, (nz, ny, nx))
+    o = OracleRun(nx, ny, nz, dx, dt, bc=(PERIODIC,) * 3)
+    o.set_potential_grid(np.zeros((nz, ny, nx))).set_state(R0, I0).set_detector(k_det, h).set_frames(True, True)
+    o.step(10).step(20)          # split across calls, not aligned with h
+    assert len(o.frames) == 1 + 30 // h
+    c = oracle.coefficients(dx, dt, 1.0, 1.0)[0]
+    kz, ky, kx = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    a = 4.0 * c * (np.sin(np.pi * kx / nx) ** 2 + np.sin(np.pi * ky / ny) ** 2 + np.sin(np.pi * kz / nz) ** 2)
+    theta = 2.0 * np.arcsin(a / 2.0)
+    r0h, i0h = np.fft.fftn(R0), np.fft.fftn(I0)
+    for f, n in enumerate(range(0, 31, h)):
+        if n == 0:
+            R, I = R0, I0
+        else:
+            with np.errstate(invalid="ignore", divide="ignore"):
+                s1 = np.where(theta > 0, np.sin(n * theta) / np.sin(theta), n)
+                s0 = np.where(theta > 0, np.sin((n - 1) * theta) / np.sin(theta), n - 1)
+            R = np.fft.ifftn((s1 * (1 - a ** 2) - s0) * r0h + s1 * a * i0h).real
+            I = np.fft.ifftn(-s1 * a * r0h + (s1 - s0) * i0h).real
+        assert rel_l2(o.frames[f], R[k_det] ** 2 + I[k_det] ** 2) < 1e-12
+    assert rel_l2(sum(o.frames[1:]), o.D) < 1e-15
+    assert np.allclose([dx * dx * f.sum() for f in o.frames[1:]], o.trace, rtol=1e-14)
+    # without the t = 0 frame the list starts at s = h
+    p = OracleRun(nx, ny, nz, dx, dt, bc=(PERIODIC,) * 3)
+    p.set_potential_grid(np.zeros((nz, ny, nx))).set_state(R0, I0).set_detector(k_det, h).set_frames(True, False).step(30)
+    assert len(p.frames) == 30 // h and np.array_equal(p.frames[0], o.frames[1])
+
+
+def test_dissimilarity_closed_forms_and_metric_properties():
+    """eq (16): closed forms that do not go through the oracle -- proportional trajectories, disjoint supports,
+    shifted Gaussians on a fine plane -- and the metric axioms (identity, symmetry, triangle inequality)."""
+    rng = np.random.default_rng(3)
+    ns, ny, nx, dA = 9, 10, 14, 0.15 ** 2
+    pattern = rng.random((ny, nx))
+    a, b = rng.random(ns) + 0.5, rng.random(ns) + 0.5
+    fa, fb = a[:, None, None] * pattern, b[:, None, None] * pattern
+    s0, s1 = 2, 7
+    # proportional frames: d = mean_s |a_s - b_s| * sqrt(dA * sum(pattern^2))
+    want = np.mean(np.abs(a - b)[s0:s1 + 1]) * math.sqrt(dA * float((pattern ** 2).sum()))
+    assert abs(oracle.dissimilarity(fa, fb, dA, s0, s1) - want) < 1e-14 * want
+    # disjoint supports: the cross term vanishes, d = mean_s sqrt(dA (|rho_k|^2 + |rho_j|^2))
+    left, right = np.zeros((ns, ny, nx)), np.zeros((ns, ny, nx))
+    left[:, :, : nx // 2] = rng.random((ns, ny, nx // 2))
+    right[:, :, nx // 2:] = rng.random((ns, ny, nx - nx // 2))
+    want = np.mean([math.sqrt(dA * float((left[s] ** 2).sum() + (right[s] ** 2).sum())) for s in range(s0, s1 + 1)])
+    assert abs(oracle.dissimilarity(left, right, dA, s0, s1) - want) < 1e-14 * want
+    # two unit Gaussians of width w a distance delta apart (continuum closed form below)
+    n, L, w, delta = 256, 16.0, 1.0, 1.3
+    x = (np.arange(n) + 0.5) * L / n
+    X, Y = np.meshgrid(x, x)
+    g1 = np.exp(-((X - 8.0) ** 2 + (Y - 8.0) ** 2) / (2 * w * w))
+    g2 = np.exp(-((X - 8.0 - delta) ** 2 + (Y - 8.0) ** 2) / (2 * w * w))
+    # int g1^2 = pi w^2, int g1 g2 = pi w^2 exp(-delta^2/(4 w^2))  =>  int (g1-g2)^2 = 2 pi w^2 (1 - exp(-delta^2/(4 w^2)))
+    want = math.sqrt(2.0 * math.pi * w * w * (1.0 - math.exp(-delta * delta / (4 * w * w))))
+    got = oracle.dissimilarity(g1[None], g2[None], (L / n) ** 2, 0, 0)
+    assert abs(got - want) < 1e-10 * want      # the trapezoid-like sum of a smooth, decayed integrand is spectrally accurate
+    # metric axioms on random trajectories
+    t = [rng.random((ns, ny, nx)) for _ in range(3)]
+    d = lambda p, q: oracle.dissimilarity(t[p], t[q], dA, 0, ns - 1)
+    assert d(0, 0) == 0.0 and d(0, 1) == d(1, 0) and d(0, 2) <= d(0, 1) + d(1, 2)
+    # scaling: rho -> alpha rho scales d by alpha
+    assert abs(oracle.dissimilarity(3.0 * t[0], 3.0 * t[1], dA, 0, ns - 1) - 3.0 * d(0, 1)) < 1e-13
