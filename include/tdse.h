@@ -145,6 +145,29 @@ int tdse_step(tdse_ctx* ctx, int n);
  * Synchronises the stream. */
 int tdse_detector_read(tdse_ctx* ctx, int b, double* image_host, double* trace_host, int cap, int* nsamples);
 
+/* Frame mode (eq (15): the paper's product is the trajectory rho = {rho(0), rho(h dt), ...} of
+ * detector-plane densities).  With max_frames > 0 every detector sample also keeps its frame
+ * rho_s[j][i] = (R^s)^2 + (I^{s-1/2})^2 in a device buffer [batch][max_frames][ny][nx] (double); with include_t0 != 0
+ * frame 0 is rho at s = 0, taken from the state in memory when tdse_step is first called, and sample s*every is
+ * frame s (else sample s*every is frame s-1).  Samples beyond max_frames are counted but not kept.  max_frames = 0
+ * turns frame mode off.  Resets image, trace, frame and step counters.  Errors: TDSE_EINVAL, TDSE_ENOMEM. */
+int tdse_set_frames(tdse_ctx* ctx, int max_frames, int include_t0);
+
+/* Copy frames first .. first+count-1 of entry b to frames_host (HOST, count*ny*nx doubles, [frame][y][x]);
+ * *nframes (may be NULL) receives the number of frames taken so far.  Synchronises.
+ * Errors: TDSE_EINVAL (entry or frame range). */
+int tdse_frames_read(tdse_ctx* ctx, int b, int first, int count, double* frames_host, int* nframes);
+
+/* Device pointer of the frame buffer (library-owned; valid until tdse_set_frames / tdse_destroy). */
+int tdse_frames_device(tdse_ctx* ctx, double** frames_device, int* max_frames, int* nframes);
+
+/* Pairwise dissimilarity of the batch entries' trajectories, eq (16) PAPER.md:219-221:
+ *   d_kj = 1/(t1-t0) int_{t0}^{t1} ( int_D (rho_k - rho_j)^2 dr )^{1/2} dt
+ * evaluated as the mean over frames first_frame .. last_frame (inclusive) of sqrt(dx^2 * sum over the plane of
+ * (rho_k - rho_j)^2) (reading 23).  d_host: HOST, batch*batch doubles, symmetric, zero diagonal.
+ * Synchronises.  Errors: TDSE_ESTATE (frame mode off), TDSE_EINVAL (window exceeds the frames kept). */
+int tdse_dissimilarity(tdse_ctx* ctx, int first_frame, int last_frame, double* d_host);
+
 /* Device pointers to the detector image [batch][ny][nx] and trace [batch][max_samples] (doubles);
  * valid until the next tdse_set_detector or tdse_destroy.  Does not synchronise. */
 int tdse_detector_device(tdse_ctx* ctx, double** image_device, double** trace_device, int* max_samples);

@@ -30,6 +30,7 @@ SYMBOLS = [
     "tdse_set_wavepacket", "tdse_set_state", "tdse_set_detector", "tdse_step",
     "tdse_detector_read", "tdse_detector_device", "tdse_read_psi", "tdse_read_potential",
     "tdse_norm", "tdse_set_option", "tdse_get_info", "tdse_last_error",
+    "tdse_set_frames", "tdse_frames_read", "tdse_frames_device", "tdse_dissimilarity",
 ]
 
 
@@ -71,6 +72,10 @@ def load():
     L.tdse_step.argtypes = [vp, C.c_int]
     L.tdse_detector_read.argtypes = [vp, C.c_int, dp, dp, C.c_int, ip]
     L.tdse_detector_device.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), ip]
+    L.tdse_set_frames.argtypes = [vp, C.c_int, C.c_int]
+    L.tdse_frames_read.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, ip]
+    L.tdse_frames_device.argtypes = [vp, C.POINTER(vp), ip, ip]
+    L.tdse_dissimilarity.argtypes = [vp, C.c_int, C.c_int, dp]
     L.tdse_read_psi.argtypes = [vp, C.c_int, vp, vp]
     L.tdse_read_potential.argtypes = [vp, C.c_int, vp]
     L.tdse_norm.argtypes = [vp, C.c_int, dp, dp]
@@ -190,6 +195,24 @@ class Tdse:
         img, tr, ms = C.c_void_p(), C.c_void_p(), C.c_int(0)
         self._check(self.L.tdse_detector_device(self._h, C.byref(img), C.byref(tr), C.byref(ms)), "tdse_detector_device")
         return img.value, tr.value, ms.value
+
+    def set_frames(self, max_frames, include_t0=True):
+        self._check(self.L.tdse_set_frames(self._h, int(max_frames), 1 if include_t0 else 0), "tdse_set_frames")
+
+    def frames_read(self, b, first=0, count=None) -> np.ndarray:
+        if count is None:
+            count = self.get_info("nframes") - first
+        out = np.empty((count, self.ny, self.nx), dtype=np.float64)
+        n = C.c_int(0)
+        self._check(self.L.tdse_frames_read(self._h, b, int(first), int(count), out.ctypes.data_as(C.POINTER(C.c_double)),
+                                            C.byref(n)), "tdse_frames_read")
+        return out
+
+    def dissimilarity(self, first_frame, last_frame) -> np.ndarray:
+        d = np.empty((self.batch, self.batch), dtype=np.float64)
+        self._check(self.L.tdse_dissimilarity(self._h, int(first_frame), int(last_frame),
+                                              d.ctypes.data_as(C.POINTER(C.c_double))), "tdse_dissimilarity")
+        return d
 
     def read_psi(self, b) -> Tuple[np.ndarray, np.ndarray]:
         R = np.empty((self.nz, self.ny, self.nx), dtype=self.np_dtype)

@@ -66,6 +66,8 @@ struct tdse_ctx {
     bool atoms_pending = false;
 
     int k_det = 0, every = 0, max_samples = 0, nsamples = 0;
+    double* frames = nullptr;           // frame mode: [batch][max_frames][ny][nx]
+    int max_frames = 0, nframes = 0, frames_t0 = 1;
     long long steps = 0;
     std::vector<char> have_V, have_state;
     double vabs_max = 0.0;
@@ -179,6 +181,7 @@ int reset_detector(tdse_ctx* c)
 {
     c->steps = 0;
     c->nsamples = 0;
+    c->nframes = 0;
     if (c->D) {
         const long long n = (long long)c->g.batch * c->g.plane;
         fill_zero_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 4096), 256, 0, c->stream>>>(c->D, n);
@@ -392,10 +395,26 @@ int sample_detector(tdse_ctx* c)
     const unsigned nblk = (unsigned)((c->g.plane + 255) / 256);
     int rc = ensure_partial(c, (size_t)nblk * c->g.batch);
     if (rc) return rc;
+    double* frame = (c->frames && c->nframes < c->max_frames) ? c->frames + (size_t)c->nframes * c->g.plane : nullptr;
     detector_accum_kernel<real><<<dim3(nblk, (unsigned)c->g.batch), 256, 0, c->stream>>>(
-        c->g, c->k_det, static_cast<const real*>(c->R[c->cur]), static_cast<const real*>(c->I[c->cur]), c->D, c->partial);
+        c->g, c->k_det, static_cast<const real*>(c->R[c->cur]), static_cast<const real*>(c->I[c->cur]), c->D, c->partial,
+        frame, (long long)c->max_frames * c->g.plane);
     CU_LAUNCH_CHECK(c);
+    if (c->frames) c->nframes++;
     return finish_trace(c, (int)nblk);
+}
+
+// frame mode: rho(0) from the state in memory before the first step
+template <typename real>
+int sample_initial_frame(tdse_ctx* c)
+{
+    const unsigned nblk = (unsigned)((c->g.plane + 255) / 256);
+    detector_accum_kernel<real><<<dim3(nblk, (unsigned)c->g.batch), 256, 0, c->stream>>>(
+        c->g, c->k_det, static_cast<const real*>(c->R[c->cur]), static_cast<const real*>(c->I[c->cur]), nullptr, nullptr,
+        c->frames, (long long)c->max_frames * c->g.plane);
+    CU_LAUNCH_CHECK(c);
+    c->nframes = 1;
+    return TDSE_OK;
 }
 
 }  // namespace
@@ -471,6 +490,7 @@ int tdse_destroy(tdse_ctx* c)
     if (c->mask_dev) cudaFree(c->mask_dev);
     if (c->D) cudaFree(c->D);
     if (c->trace) cudaFree(c->trace);
+    if (c->frames) cudaFree(c->frames);
     if (c->partial) cudaFree(c->partial);
     if (c->scalars) cudaFree(c->scalars);
     if (c->atoms_dev) cudaFree(c->atoms_dev);
@@ -681,6 +701,10 @@ int tdse_step(tdse_ctx* c, int n)
         return fail(c, TDSE_EINVAL, "tdse_step: fused kernel needs a 5-array workspace, rows of whole 16-byte groups, even ny, nx >= 8 and ny >= 8");
     const int tmax = (c->opt_tblock > 0) ? c->opt_tblock : 2;
     c->last_kernel = kernel;
+    if (n > 0 && c->frames && c->frames_t0 && c->every > 0 && c->steps == 0 && c->nframes == 0) {
+        const int rc0 = (c->dtype == TDSE_F32) ? sample_initial_frame<float>(c) : sample_initial_frame<double>(c);
+        if (rc0) return rc0;
+    }
     int remaining = n;
     while (remaining > 0) {
         const int to_sample = (c->every > 0) ? (int)(c->every - (c->steps % c->every)) : std::numeric_limits<int>::max();
@@ -730,6 +754,70 @@ int tdse_detector_read(tdse_ctx* c, int b, double* image_host, double* trace_hos
         CU_TRY(c, cudaMemcpyAsync(trace_host, c->trace + (size_t)b * c->max_samples, (size_t)ntr * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     if (nsamples) *nsamples = c->nsamples;
+    return TDSE_OK;
+}
+
+int tdse_set_frames(tdse_ctx* c, int max_frames, int include_t0)
+{
+    if (!c) return TDSE_EINVAL;
+    if (max_frames < 0) return fail(c, TDSE_EINVAL, "tdse_set_frames: max_frames < 0");
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    if (c->frames) { cudaFree(c->frames); c->frames = nullptr; }
+    c->max_frames = 0; c->frames_t0 = include_t0 ? 1 : 0;
+    if (max_frames > 0) {
+        cudaError_t e = cudaMalloc(&c->frames, (size_t)c->g.batch * max_frames * c->g.plane * sizeof(double));
+        if (e != cudaSuccess) { cudaGetLastError(); c->frames = nullptr; return fail(c, TDSE_ENOMEM, std::string("tdse_set_frames: ") + cudaGetErrorString(e)); }
+        c->max_frames = max_frames;
+    }
+    return reset_detector(c);
+}
+
+int tdse_frames_read(tdse_ctx* c, int b, int first, int count, double* frames_host, int* nframes)
+{
+    if (!c) return TDSE_EINVAL;
+    if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_frames_read: entry out of range");
+    const int have = std::min(c->nframes, c->max_frames);
+    if (first < 0 || count < 0 || first + count > have) return fail(c, TDSE_EINVAL, "tdse_frames_read: frame range exceeds the frames kept");
+    if (count > 0) {
+        if (!frames_host) return fail(c, TDSE_EINVAL, "tdse_frames_read: NULL");
+        CU_TRY(c, cudaMemcpyAsync(frames_host, c->frames + ((size_t)b * c->max_frames + first) * c->g.plane,
+                                  (size_t)count * c->g.plane * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    }
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    if (nframes) *nframes = c->nframes;
+    return TDSE_OK;
+}
+
+int tdse_frames_device(tdse_ctx* c, double** frames_device, int* max_frames, int* nframes)
+{
+    if (!c) return TDSE_EINVAL;
+    if (frames_device) *frames_device = c->frames;
+    if (max_frames) *max_frames = c->max_frames;
+    if (nframes) *nframes = c->nframes;
+    return TDSE_OK;
+}
+
+int tdse_dissimilarity(tdse_ctx* c, int first_frame, int last_frame, double* d_host)
+{
+    if (!c) return TDSE_EINVAL;
+    if (!d_host) return fail(c, TDSE_EINVAL, "tdse_dissimilarity: NULL");
+    if (!c->frames) return fail(c, TDSE_ESTATE, "tdse_dissimilarity: frame mode is off (tdse_set_frames)");
+    const int have = std::min(c->nframes, c->max_frames);
+    if (first_frame < 0 || last_frame < first_frame || last_frame >= have)
+        return fail(c, TDSE_EINVAL, "tdse_dissimilarity: frame window exceeds the frames kept");
+    const int nwin = last_frame - first_frame + 1, batch = c->g.batch;
+    int rc = ensure_partial(c, (size_t)batch * batch * nwin + (size_t)batch * batch);
+    if (rc) return rc;
+    double* inner = c->partial;
+    double* d_dev = c->partial + (size_t)batch * batch * nwin;
+    const int tiles = (batch + kDisTile - 1) / kDisTile;
+    dissimilarity_inner_kernel<<<dim3((unsigned)(tiles * tiles), (unsigned)nwin), 256, 0, c->stream>>>(
+        c->frames, batch, (long long)c->max_frames * c->g.plane, (int)c->g.plane, c->dx * c->dx, first_frame, nwin, inner);
+    CU_LAUNCH_CHECK(c);
+    dissimilarity_finish_kernel<<<(batch * batch + 127) / 128, 128, 0, c->stream>>>(inner, batch, nwin, d_dev);
+    CU_LAUNCH_CHECK(c);
+    CU_TRY(c, cudaMemcpyAsync(d_host, d_dev, (size_t)batch * batch * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
     return TDSE_OK;
 }
 
@@ -827,6 +915,7 @@ int tdse_get_info(const tdse_ctx* c, const char* key, long long* value)
     else if (k == "tile_y") *value = c->last_tile_y;
     else if (k == "z_chunks") *value = c->last_chunks;
     else if (k == "nsamples") *value = c->nsamples;
+    else if (k == "nframes") *value = c->nframes;
     else return TDSE_EINVAL;
     return TDSE_OK;
 }

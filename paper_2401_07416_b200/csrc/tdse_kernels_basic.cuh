@@ -210,13 +210,15 @@ half_step_kernel(Grid g, real c, real cv, real sgn, const real* __restrict__ V,
 
 // ---------------------------------------------------------------------------------------------
 // S5 detector (eq (15), density of PAPER.md:87): D += R^2 + I^2 on plane k_det,
-// per-block partial sums (double) -> trace_finish_kernel sums them in fixed order.
-// grid: x = ceil(nx*ny / 256), y = batch.
+// per-block partial sums (double) -> trace_finish_kernel sums them in fixed order.  Frame mode (the
+// trajectory rho = {rho(0), rho(h dt), ...}) also keeps the sampled plane: frame[b][p] = rho.  D, partial and
+// frame may each be NULL (frame-only call for rho(0)).  grid: x = ceil(nx*ny / 256), y = batch.
 // ---------------------------------------------------------------------------------------------
 template <typename real>
 __global__ void __launch_bounds__(256)
 detector_accum_kernel(Grid g, int k_det, const real* __restrict__ R, const real* __restrict__ I,
-                      double* __restrict__ D, double* __restrict__ partial /* [batch][gridDim.x] */)
+                      double* __restrict__ D, double* __restrict__ partial /* [batch][gridDim.x] */,
+                      double* __restrict__ frame /* this sample's frame of entry 0 */, long long frame_entry_stride)
 {
     __shared__ double scratch[32];
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -225,10 +227,77 @@ detector_accum_kernel(Grid g, int k_det, const real* __restrict__ R, const real*
         const long long off = (long long)blockIdx.y * g.pcells + cell_offset(g, (int)(p % g.nx), (int)(p / g.nx), k_det);
         const double r = (double)R[off], im = (double)I[off];
         rho = r * r + im * im;
-        D[(long long)blockIdx.y * g.plane + p] += rho;
+        if (D) D[(long long)blockIdx.y * g.plane + p] += rho;
+        if (frame) frame[(long long)blockIdx.y * frame_entry_stride + p] = rho;
     }
-    const double s = block_sum(rho, scratch);
-    if (threadIdx.x == 0) partial[(long long)blockIdx.y * gridDim.x + blockIdx.x] = s;
+    if (partial) {
+        const double s = block_sum(rho, scratch);
+        if (threadIdx.x == 0) partial[(long long)blockIdx.y * gridDim.x + blockIdx.x] = s;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Trajectory dissimilarity, eq (16), over the batch entries of one context:
+//   d_kj = mean over frames s0..s1 of sqrt( dA * sum_p (rho_k[s][p] - rho_j[s][p])^2 )      (reading 23)
+// A block takes a kDisTile x kDisTile tile of entry pairs and one frame, so every frame it reads serves
+// kDisTile pairs; fixed-order block sums (deterministic).  inner[(k*batch + j)*nwin + s-s0] = sqrt(dA * sum).
+// grid: x = tiles_k * tiles_j, y = nwin.
+// ---------------------------------------------------------------------------------------------
+constexpr int kDisTile = 4;
+
+__global__ void __launch_bounds__(256)
+dissimilarity_inner_kernel(const double* __restrict__ frames, int batch, long long entry_stride, int npix,
+                           double dA, int s0, int nwin, double* __restrict__ inner)
+{
+    __shared__ double scratch[32];
+    const int tiles = (batch + kDisTile - 1) / kDisTile;
+    const int tk = blockIdx.x / tiles, tj = blockIdx.x % tiles;
+    if (tj < tk) return;                              // d is symmetric: upper triangle of tiles only
+    const int s = blockIdx.y;
+    const double* fk[kDisTile];
+    const double* fj[kDisTile];
+#pragma unroll
+    for (int q = 0; q < kDisTile; ++q) {
+        fk[q] = frames + (long long)min(tk * kDisTile + q, batch - 1) * entry_stride + (long long)(s0 + s) * npix;
+        fj[q] = frames + (long long)min(tj * kDisTile + q, batch - 1) * entry_stride + (long long)(s0 + s) * npix;
+    }
+    double acc[kDisTile][kDisTile];
+#pragma unroll
+    for (int a = 0; a < kDisTile; ++a)
+#pragma unroll
+        for (int b = 0; b < kDisTile; ++b) acc[a][b] = 0.0;
+    for (int p = threadIdx.x; p < npix; p += blockDim.x) {
+        double vk[kDisTile], vj[kDisTile];
+#pragma unroll
+        for (int q = 0; q < kDisTile; ++q) { vk[q] = fk[q][p]; vj[q] = fj[q][p]; }
+#pragma unroll
+        for (int a = 0; a < kDisTile; ++a)
+#pragma unroll
+            for (int b = 0; b < kDisTile; ++b) { const double d = vk[a] - vj[b]; acc[a][b] = fma(d, d, acc[a][b]); }
+    }
+#pragma unroll
+    for (int a = 0; a < kDisTile; ++a)
+#pragma unroll
+        for (int b = 0; b < kDisTile; ++b) {
+            const double t = block_sum(acc[a][b], scratch);
+            const int k = tk * kDisTile + a, j = tj * kDisTile + b;
+            if (threadIdx.x == 0 && k < batch && j < batch)
+                inner[((long long)k * batch + j) * nwin + s] = sqrt(dA * t);
+        }
+}
+
+// d[k][j] = d[j][k] = mean_s inner[k][j][s] for k <= j (serial over frames, fixed order).  One thread per pair.
+__global__ void dissimilarity_finish_kernel(const double* __restrict__ inner, int batch, int nwin, double* __restrict__ d)
+{
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= batch * batch) return;
+    const int k = q / batch, j = q % batch;
+    if (j < k) return;
+    double acc = 0.0;
+    for (int s = 0; s < nwin; ++s) acc += inner[((long long)k * batch + j) * nwin + s];
+    const double v = (k == j) ? 0.0 : acc / (double)nwin;
+    d[(long long)k * batch + j] = v;
+    d[(long long)j * batch + k] = v;
 }
 
 // trace[b][slot] = scale * sum_{q < nparts} partial[b][q]  (serial, fixed order).  One thread per entry.

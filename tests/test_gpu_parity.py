@@ -240,6 +240,57 @@ def test_config4_reduced_grid_fp32_vs_fp64_detector_agreement():
 
 
 # ------------------------------------------------------------------------------------------
+# frame-mode detector and pairwise dissimilarity (eq 16)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("include_t0", [True, False])
+def test_frames_and_dissimilarity_match_oracle(dtype, include_t0):
+    from paper_2401_07416_b200 import Tdse, TdseError, TDSE_EINVAL, TDSE_ESTATE
+    w = make_config(3, n=(40, 36, 44), batch=5, steps=46, dtype=dtype)     # 5 entries: a full 4x4 pair tile + a ragged one
+    w = w.with_(every=5)
+    t = Tdse.from_workload(w)
+    with pytest.raises(TdseError) as e:                    # frame mode is off
+        t.dissimilarity(0, 1)
+    assert e.value.code == TDSE_ESTATE
+    nfr = w.steps // w.every + (1 if include_t0 else 0)
+    t.set_frames(nfr + 3, include_t0)
+    t.step(17)
+    t.step(w.steps - 17)                                   # split across calls, not aligned with the sampling period
+    assert t.get_info("nframes") == nfr
+    tol = TOL[dtype]
+    ora, gpu = [], []
+    for b in range(w.batch):
+        o = OracleRun.from_workload(w, entry=b, dtype="f64", round_to="f32" if dtype == "f32" else None)
+        o.set_frames(True, include_t0).step(w.steps)
+        fr = t.frames_read(b)
+        assert fr.shape == (nfr, w.ny, w.nx) and len(o.frames) == nfr
+        for s in range(nfr):
+            assert rel_l2(fr[s], o.frames[s]) < tol
+        D, tr = t.detector_read(b)
+        first = 1 if include_t0 else 0
+        assert rel_l2(fr[first:].sum(axis=0), D) < 1e-14   # the accumulated image is the sum of the kept frames
+        assert np.allclose(w.dx ** 2 * fr[first:].sum(axis=(1, 2)), tr, rtol=1e-12)
+        ora.append(np.array(o.frames)); gpu.append(fr)
+    s0, s1 = 2, nfr - 2
+    d = t.dissimilarity(s0, s1)
+    assert d.shape == (5, 5) and np.array_equal(d, d.T) and np.all(np.diag(d) == 0.0)
+    for k in range(w.batch):
+        for j in range(k + 1, w.batch):
+            # the reduction alone (same frames in, different summation order): rounding level
+            assert abs(d[k, j] - oracle.dissimilarity(gpu[k], gpu[j], w.dx ** 2, s0, s1)) <= 1e-12 * d[k, j]
+            # end to end against the oracle's own trajectories
+            want = oracle.dissimilarity(ora[k], ora[j], w.dx ** 2, s0, s1)
+            assert abs(d[k, j] - want) <= 10 * tol * want
+    with pytest.raises(TdseError) as e:
+        t.dissimilarity(0, nfr)                            # window beyond the frames kept
+    assert e.value.code == TDSE_EINVAL
+    with pytest.raises(TdseError) as e:
+        t.frames_read(0, nfr - 1, 2)
+    assert e.value.code == TDSE_EINVAL
+    t.close()
+
+
+# ------------------------------------------------------------------------------------------
 # edge cases and error behaviour of the boundary
 # ------------------------------------------------------------------------------------------
 def test_call_order_and_stability_errors():
