@@ -533,8 +533,10 @@ static int build_potential(tdse_ctx* c, int b, const AtomRec* atoms_dev, int nat
 {
     int b0, b1;
     if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_potential: entry out of range");
-    const long long pot_slots = (long long)((c->g.nx + kPotCells - 1) / kPotCells) * c->g.ny * c->g.nz;
-    const unsigned nblk = (unsigned)((pot_slots + 255) / 256);
+    const long long pot_bricks = (long long)((c->g.nx + kPotCells * kPotBX - 1) / (kPotCells * kPotBX)) *
+                                 ((c->g.ny + kPotBY - 1) / kPotBY) * ((c->g.nz + kPotBZ - 1) / kPotBZ);
+    if (pot_bricks > 0x7fffffffLL) return fail(c, TDSE_EINVAL, "tdse_set_potential: grid too large");
+    const unsigned nblk = (unsigned)pot_bricks;
     void* dst = entry_ptr(c, c->V, b0);
     if (c->dtype == TDSE_F32)
         potential_build_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->dx, atoms_dev, natoms, vmin, vmax, rcut, static_cast<float*>(dst));

@@ -48,40 +48,73 @@ __device__ __forceinline__ double exp_nonpositive(double x)
     return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));   // p * 2^k, k >= -1022
 }
 
+// distance from coordinate a to the interval [lo, hi] along one axis (nearest periodic image if L > 0)
+__device__ __forceinline__ double axis_gap(double a, double lo, double hi, double L)
+{
+    double g = fmax(0.0, fmax(lo - a, a - hi));
+    if (L > 0.0) {
+        g = fmin(g, fmax(0.0, fmax(lo - (a + L), (a + L) - hi)));
+        g = fmin(g, fmax(0.0, fmax(lo - (a - L), (a - L) - hi)));
+    }
+    return g;
+}
+
+// A block owns a brick of kPotBX x kPotBY x kPotBZ threads = (4 kPotBX) x kPotBY x kPotBZ cells.  With a cutoff, atoms
+// farther than rcut from every cell of the brick are dropped while the list is staged (ordered compaction, so
+// the summation order of the kept atoms is the list order); per pair the cutoff test itself is unchanged.
+constexpr int kPotBX = 16, kPotBY = 4, kPotBZ = 4;
+
 template <typename real>
 __global__ void __launch_bounds__(256)
 potential_build_kernel(Grid g, double dx, const AtomRec* __restrict__ atoms, int natoms,
                        double vmin, double vmax, double rcut, real* __restrict__ V /* entry base */)
 {
+    static_assert(kPotBX * kPotBY * kPotBZ == 256 && kAtomChunk <= 256, "block shape");
     __shared__ AtomStaged s_atoms[kAtomChunk];
-    const int nxq = (g.nx + kPotCells - 1) / kPotCells;
-    const long long slot = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = slot < (long long)nxq * g.ny * g.nz;
-    int i0 = 0, j = 0, k = 0;
-    if (live) {
-        i0 = (int)(slot % nxq) * kPotCells;
-        const long long t = slot / nxq;
-        j = (int)(t % g.ny);
-        k = (int)(t / g.ny);
-    }
+    __shared__ int s_warp_count[8];
+    const int tx = threadIdx.x % kPotBX, ty = (threadIdx.x / kPotBX) % kPotBY, tz = threadIdx.x / (kPotBX * kPotBY);
+    const int bricks_x = (g.nx + kPotCells * kPotBX - 1) / (kPotCells * kPotBX), bricks_y = (g.ny + kPotBY - 1) / kPotBY;
+    const int bx = blockIdx.x % bricks_x, by = (blockIdx.x / bricks_x) % bricks_y, bz = blockIdx.x / (bricks_x * bricks_y);
+    const int i0 = (bx * kPotBX + tx) * kPotCells, j = by * kPotBY + ty, k = bz * kPotBZ + tz;
+    const bool live = i0 < g.nx && j < g.ny && k < g.nz;
     const double y = j * dx, z = k * dx;
     const double Lx = g.nx * dx, Ly = g.ny * dx, Lz = g.nz * dx;
     const double iLx = 1.0 / Lx, iLy = 1.0 / Ly, iLz = 1.0 / Lz;
     const bool perx = g.bcx == BC_PERIODIC, pery = g.bcy == BC_PERIODIC, perz = g.bcz == BC_PERIODIC;
     const double rc2 = rcut * rcut;
+    // the brick's bounding box, padded by a cell so that rounding never drops an atom the pair test would keep
+    const double lox = (bx * kPotBX * kPotCells - 1) * dx, hix = ((bx + 1) * kPotBX * kPotCells) * dx;
+    const double loy = (by * kPotBY - 1) * dx, hiy = ((by + 1) * kPotBY) * dx;
+    const double loz = (bz * kPotBZ - 1) * dx, hiz = ((bz + 1) * kPotBZ) * dx;
     double sum[kPotCells];
 #pragma unroll
     for (int e = 0; e < kPotCells; ++e) sum[e] = 0.0;
     for (int a0 = 0; a0 < natoms; a0 += kAtomChunk) {
-        const int na = min(kAtomChunk, natoms - a0);
-        __syncthreads();
-        for (int q = threadIdx.x; q < na; q += blockDim.x) {
-            const AtomRec A = atoms[a0 + q];
-            AtomStaged S;
+        const int nc = min(kAtomChunk, natoms - a0);
+        __syncthreads();                                  // previous chunk fully consumed
+        // ---- stage: thread q < nc looks at atom a0 + q; kept atoms are compacted in list order ----
+        AtomStaged S;
+        bool keep = false;
+        if (threadIdx.x < nc) {
+            const AtomRec A = atoms[a0 + threadIdx.x];
             S.x = A.x; S.y = A.y; S.z = A.z; S.Z = A.Z; S.soft2 = A.soft2;
             S.inv_screen = (A.screen > 0.0 && isfinite(A.screen)) ? 1.0 / A.screen : 0.0;
-            s_atoms[q] = S;
+            keep = true;
+            if (rcut > 0.0) {
+                const double gx = axis_gap(A.x, lox, hix, perx ? Lx : 0.0);
+                const double gy = axis_gap(A.y, loy, hiy, pery ? Ly : 0.0);
+                const double gz = axis_gap(A.z, loz, hiz, perz ? Lz : 0.0);
+                keep = gx * gx + gy * gy + gz * gz <= rc2;
+            }
         }
+        const unsigned ballot = __ballot_sync(0xffffffffu, keep);
+        const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        if (lane == 0) s_warp_count[warp] = __popc(ballot);
+        __syncthreads();
+        int base = 0, na = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) { if (w < warp) base += s_warp_count[w]; na += s_warp_count[w]; }
+        if (keep) s_atoms[base + __popc(ballot & ((1u << lane) - 1u))] = S;
         __syncthreads();
         if (!live) continue;
         for (int a = 0; a < na; ++a) {
