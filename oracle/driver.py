@@ -43,10 +43,10 @@ def lib():
             dp, fp, ip = C.POINTER(C.c_double), C.POINTER(C.c_float), C.POINTER(C.c_int)
             L.oracle_max_threads.restype = C.c_int
             L.oracle_set_threads.argtypes = [C.c_int]
-            L.oracle_potential.argtypes = [C.c_int] * 3 + [C.c_double] + [C.c_int] * 3 + \
+            L.oracle_potential.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [C.c_int] * 3 + \
                 [dp, C.c_int, C.c_double, C.c_double, C.c_double, dp]
             L.oracle_mask.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, dp]
-            L.oracle_wavepacket.argtypes = [C.c_int] * 3 + [C.c_double] * 9 + [dp, dp]
+            L.oracle_wavepacket.argtypes = [C.c_int] * 3 + [C.c_double] * 11 + [dp, dp]
             L.oracle_stagger.argtypes = [C.c_int] * 6 + [C.c_double] * 4 + [dp, dp, dp, dp]
             for sfx, rp in (("f64", dp), ("f32", fp)):
                 f = getattr(L, "oracle_step_" + sfx)
@@ -97,10 +97,12 @@ def paper_wavelength(energy: float, mass: float, hbar: float) -> float:
     return float(np.sqrt(2.0 * hbar * hbar * np.pi ** 2 / (mass * energy)))
 
 
-def potential(nx, ny, nz, dx, bc, atoms, vmin, vmax, rcut=0.0) -> np.ndarray:
+def potential(nx, ny, nz, dx, bc, atoms, vmin, vmax, rcut=0.0, dy=None, dz=None) -> np.ndarray:
     atoms = np.ascontiguousarray(np.asarray(atoms, dtype=np.float64).reshape(-1, 6))
     V = np.empty((nz, ny, nx), dtype=np.float64)
-    lib().oracle_potential(nx, ny, nz, dx, bc[0], bc[1], bc[2], _p(atoms, C.c_double),
+    dy = dx if dy is None else dy
+    dz = dx if dz is None else dz
+    lib().oracle_potential(nx, ny, nz, dx, dy, dz, bc[0], bc[1], bc[2], _p(atoms, C.c_double),
                            atoms.shape[0], vmin, vmax, rcut, _p(V, C.c_double))
     return V
 
@@ -111,10 +113,12 @@ def mask(nz, w_lo, w_hi, strength=0.05, power=2) -> np.ndarray:
     return M
 
 
-def wavepacket(nx, ny, nz, dx, x0, y0, z0, sigma, kx, ky, kz, amplitude=0.0):
+def wavepacket(nx, ny, nz, dx, x0, y0, z0, sigma, kx, ky, kz, amplitude=0.0, dy=None, dz=None):
     R0 = np.empty((nz, ny, nx), dtype=np.float64)
     J0 = np.empty((nz, ny, nx), dtype=np.float64)
-    lib().oracle_wavepacket(nx, ny, nz, dx, x0, y0, z0, sigma, kx, ky, kz, amplitude,
+    dy = dx if dy is None else dy
+    dz = dx if dz is None else dz
+    lib().oracle_wavepacket(nx, ny, nz, dx, dy, dz, x0, y0, z0, sigma, kx, ky, kz, amplitude,
                             _p(R0, C.c_double), _p(J0, C.c_double))
     return R0, J0
 
@@ -148,15 +152,17 @@ class OracleRun:
 
     def __init__(self, nx, ny, nz, dx, dt, mass=1.0, hbar=1.0, dtype="f64",
                  bc=(DIRICHLET, DIRICHLET, DIRICHLET), absorb_lo=0, absorb_hi=0,
-                 strength=0.05, power=2, round_to: Optional[str] = None):
+                 strength=0.05, power=2, round_to: Optional[str] = None, dy=None, dz=None):
         assert dtype in ("f64", "f32")
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.dx, self.dt, self.mass, self.hbar = float(dx), float(dt), float(mass), float(hbar)
+        self.dy = self.dx if dy is None else float(dy)       # anisotropic mesh of the paper
+        self.dz = self.dx if dz is None else float(dz)
         self.dtype = dtype
         self.np = np.float64 if dtype == "f64" else np.float32
         self.round_to = round_to if round_to else dtype
         self.bc = tuple(int(b) for b in bc)
-        coef = coefficients(dx, dt, mass, hbar)
+        coef = coefficients(dx, dt, mass, hbar, self.dy, self.dz)
         self.coef = tuple(self._round_scalar(c) for c in coef)
         self.M = self._round(mask(self.nz, absorb_lo, absorb_hi, strength, power))
         self.V = None
@@ -181,7 +187,7 @@ class OracleRun:
 
     # -- inputs ---------------------------------------------------------------------
     def set_potential_atoms(self, atoms, vmin, vmax, rcut=0.0):
-        self.V64 = potential(self.nx, self.ny, self.nz, self.dx, self.bc, atoms, vmin, vmax, rcut)
+        self.V64 = potential(self.nx, self.ny, self.nz, self.dx, self.bc, atoms, vmin, vmax, rcut, self.dy, self.dz)
         self.V = self._round(self.V64)
         return self
 
@@ -192,8 +198,8 @@ class OracleRun:
 
     def set_wavepacket(self, x0, y0, z0, sigma, kx, ky, kz, amplitude=0.0):
         assert self.V is not None, "potential first (the staggered start needs V)"
-        R0, J0 = wavepacket(self.nx, self.ny, self.nz, self.dx, x0, y0, z0, sigma, kx, ky, kz, amplitude)
-        Ih = stagger(self.bc, coefficients(self.dx, self.dt, self.mass, self.hbar),
+        R0, J0 = wavepacket(self.nx, self.ny, self.nz, self.dx, x0, y0, z0, sigma, kx, ky, kz, amplitude, self.dy, self.dz)
+        Ih = stagger(self.bc, coefficients(self.dx, self.dt, self.mass, self.hbar, self.dy, self.dz),
                      self.V.astype(np.float64), R0, J0)
         self.R, self.I = self._round(R0), self._round(Ih)
         self.counter = C.c_longlong(0)
@@ -250,7 +256,7 @@ class OracleRun:
         ns = C.c_int(0)
         f(self.nx, self.ny, self.nz, *self.bc, *self.coef,
           _p(self.V, ct), _p(self.M, ct), _p(self.R, ct), _p(self.I, ct), int(n),
-          C.byref(self.counter), self.k_det, self.every, self.dx,
+          C.byref(self.counter), self.k_det, self.every, self.dx * self.dy,
           _p(self.D, C.c_double), _p(tr, C.c_double), cap, C.byref(ns))
         self.trace.extend(tr[: ns.value].tolist())
         return self
@@ -259,7 +265,7 @@ class OracleRun:
         ct = C.c_double if self.dtype == "f64" else C.c_float
         g = getattr(lib(), "oracle_norm_" + self.dtype)
         qv, qp = C.c_double(0), C.c_double(0)
-        g(self.nx, self.ny, self.nz, *self.bc, *self.coef, self.dx,
+        g(self.nx, self.ny, self.nz, *self.bc, *self.coef, self.dx * self.dy * self.dz,
           _p(self.V, ct), _p(self.M, ct), _p(self.R, ct), _p(self.I, ct), C.byref(qv), C.byref(qp))
         return qv.value, qp.value
 
@@ -268,7 +274,8 @@ class OracleRun:
                       round_to: Optional[str] = None) -> "OracleRun":
         """Set up batch entry `entry` of a workloads.Workload (inputs only; no stepping)."""
         o = cls(w.nx, w.ny, w.nz, w.dx, w.dt, w.mass, w.hbar, dtype or w.dtype, w.bc,
-                w.absorb_lo, w.absorb_hi, w.strength, w.power, round_to=round_to)
+                w.absorb_lo, w.absorb_hi, w.strength, w.power, round_to=round_to,
+                dy=getattr(w, "dy", None), dz=getattr(w, "dz", None))
         o.set_potential_atoms(w.atoms[entry], w.vmin, w.vmax, w.rcut)
         o.set_wavepacket(**w.packet)
         o.set_detector(w.k_det, w.every)

@@ -58,21 +58,21 @@ void oracle_set_threads(int n)
 
 /* V(i,j,k) = clamp( sum_a -Z_a * screen_a(r_a) / sqrt(r_a^2 + s_a^2), vmin, vmax )
  * atoms: natoms records (x, y, z, Z, s^2, lambda); lambda <= 0 or non-finite: screen = 1.
- * r_a: distance from the grid point (i dx, j dx, k dx) to the atom; on a
+ * r_a: distance from the grid point (i dx, j dy, k dz) to the atom; on a
  * periodic axis the displacement is reduced to the nearest image, d <- d - L round(d/L).
  * rcut > 0: atoms with r_a > rcut are skipped.  Sum in list order, double throughout. */
-void oracle_potential(int nx, int ny, int nz, double dx, int bcx, int bcy, int bcz,
+void oracle_potential(int nx, int ny, int nz, double dx, double dy, double dz, int bcx, int bcy, int bcz,
                       const double* atoms, int natoms, double vmin, double vmax, double rcut,
                       double* V)
 {
-    const double Lx = nx * dx, Ly = ny * dx, Lz = nz * dx;
+    const double Lx = nx * dx, Ly = ny * dy, Lz = nz * dz;
 #ifdef _OPENMP
 #pragma omp parallel for schedule(static)
 #endif
     for (int k = 0; k < nz; ++k)
         for (int j = 0; j < ny; ++j)
             for (int i = 0; i < nx; ++i) {
-                const double x = i * dx, y = j * dx, z = k * dx;
+                const double x = i * dx, y = j * dy, z = k * dz;
                 double sum = 0.0;
                 for (int a = 0; a < natoms; ++a) {
                     const double* A = atoms + 6 * (size_t)a;
@@ -110,7 +110,7 @@ void oracle_mask(int nz, int w_lo, int w_hi, double strength, int power, double*
 /* psi0 = N exp(-|r - r0|^2 / (2 sigma^2)) exp(+i k0.(r - r0)), eq (3) with the paper's
  * case k0 = (0, 0, -2 pi / lambda).  amplitude == 0: N = (pi sigma^2)^(-3/4).
  * Outputs R0 = Re psi0, J0 = Im psi0 (double). */
-void oracle_wavepacket(int nx, int ny, int nz, double dx,
+void oracle_wavepacket(int nx, int ny, int nz, double dx, double dy, double dz,
                        double x0, double y0, double z0, double sigma,
                        double kx, double ky, double kz, double amplitude,
                        double* R0, double* J0)
@@ -120,7 +120,7 @@ void oracle_wavepacket(int nx, int ny, int nz, double dx,
     for (int k = 0; k < nz; ++k)
         for (int j = 0; j < ny; ++j)
             for (int i = 0; i < nx; ++i) {
-                const double ddx = i * dx - x0, ddy = j * dx - y0, ddz = k * dx - z0;
+                const double ddx = i * dx - x0, ddy = j * dy - y0, ddz = k * dz - z0;
                 const double G = N * exp(-(ddx * ddx + ddy * ddy + ddz * ddz) / (2.0 * sigma * sigma));
                 const double phi = kx * ddx + ky * ddy + kz * ddz;
                 const size_t p = ((size_t)k * ny + j) * nx + i;

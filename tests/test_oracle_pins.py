@@ -492,3 +492,64 @@ def test_dissimilarity_closed_forms_and_metric_properties():
     assert d(0, 0) == 0.0 and d(0, 1) == d(1, 0) and d(0, 2) <= d(0, 1) + d(1, 2)
     # scaling: rho -> alpha rho scales d by alpha
     assert abs(oracle.dissimilarity(3.0 * t[0], 3.0 * t[1], dA, 0, ns - 1) - 3.0 * d(0, 1)) < 1e-13
+
+
+# ---------------------------------------------------------------------------------------
+# anisotropic mesh (c_x != c_y != c_z; the paper's own mesh is 35.4/240 x 40.9/240 x 70/420 A)
+# ---------------------------------------------------------------------------------------
+def test_anisotropic_recurrence_vs_dense_and_fft_closed_forms():
+    # tiny mixed-BC grid: dense A with one coefficient per axis, built here with numpy
+    nx, ny, nz = 5, 4, 6
+    bc = (PERIODIC, DIRICHLET, PERIODIC)
+    dx, dy, dz, dt = 0.4, 0.3, 0.55, 0.004
+    V = random_potential(21, (nz, ny, nx), -3.0, 1.0)
+    R0, I0 = random_state(22, (nz, ny, nx))
+    o = OracleRun(nx, ny, nz, dx, dt, bc=bc, dy=dy, dz=dz).set_potential_grid(V).set_state(R0, I0)
+    n = 150
+    o.step(n)
+    cx, cy, cz, cv = oracle.coefficients(dx, dt, 1.0, 1.0, dy, dz)
+    assert cx != cy != cz
+    Ix, Iy, Iz = np.eye(nx), np.eye(ny), np.eye(nz)
+    A = (-cz * np.kron(np.kron(d2_matrix(nz, bc[2]), Iy), Ix) - cy * np.kron(np.kron(Iz, d2_matrix(ny, bc[1])), Ix)
+         - cx * np.kron(np.kron(Iz, Iy), d2_matrix(nx, bc[0])) + cv * np.diag(V.ravel()))
+    a, U = np.linalg.eigh(A)
+    r, i = leapfrog_modes(a, U.T @ R0.ravel(), U.T @ I0.ravel(), n)
+    assert rel_l2(o.R, U @ r) < 1e-12 and rel_l2(o.I, U @ i) < 1e-12
+    # medium periodic free grid: Fourier symbol a = sum_d 4 c_d sin^2(pi kappa_d / n_d)
+    nx, ny, nz = 16, 12, 20
+    R0, I0 = random_state(23, (nz, ny, nx))
+    o = OracleRun(nx, ny, nz, dx, dt, bc=(PERIODIC,) * 3, dy=dy, dz=dz)
+    o.set_potential_grid(np.zeros((nz, ny, nx))).set_state(R0, I0).set_detector(3, 10)
+    n = 120
+    o.step(n)
+    kz, ky, kx = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    a = 4.0 * (cx * np.sin(np.pi * kx / nx) ** 2 + cy * np.sin(np.pi * ky / ny) ** 2 + cz * np.sin(np.pi * kz / nz) ** 2)
+    theta = 2.0 * np.arcsin(a / 2.0)
+    with np.errstate(invalid="ignore", divide="ignore"):
+        s1 = np.where(theta > 0, np.sin(n * theta) / np.sin(theta), n)
+        s0 = np.where(theta > 0, np.sin((n - 1) * theta) / np.sin(theta), n - 1)
+    r0h, i0h = np.fft.fftn(R0), np.fft.fftn(I0)
+    R = np.fft.ifftn((s1 * (1 - a ** 2) - s0) * r0h + s1 * a * i0h).real
+    I = np.fft.ifftn(-s1 * a * r0h + (s1 - s0) * i0h).real
+    assert rel_l2(o.R, R) < 1e-12 and rel_l2(o.I, I) < 1e-12
+    # the trace carries the plane's area element dx*dy, the norms the volume element dx*dy*dz
+    assert abs(o.trace[-1] - dx * dy * float((R[3] ** 2 + I[3] ** 2).sum())) < 1e-12 * o.trace[-1]
+    qv, qp = o.norm()
+    assert abs(qp - dx * dy * dz * float((R ** 2 + I ** 2).sum())) < 1e-12 * qp
+
+
+def test_anisotropic_potential_and_packet_closed_forms():
+    nx, ny, nz, dx, dy, dz = 12, 10, 14, 0.3, 0.2, 0.45
+    atom = np.array([[1.1, 0.7, 2.9, 3.0, 0.2, 0.8]])
+    V = oracle.potential(nx, ny, nz, dx, (DIRICHLET,) * 3, atom, -1e9, 0.0, dy=dy, dz=dz)
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    r = np.sqrt((i * dx - 1.1) ** 2 + (j * dy - 0.7) ** 2 + (k * dz - 2.9) ** 2)
+    assert np.allclose(V, -3.0 * np.exp(-r / 0.8) / np.sqrt(r * r + 0.2), rtol=1e-13)
+    # nearest image uses the box lengths n_d * d_d of each axis
+    Vp = oracle.potential(nx, ny, nz, dx, (PERIODIC,) * 3, atom, -1e9, 0.0, dy=dy, dz=dz)
+    shifted = atom + np.array([[nx * dx, -ny * dy, 2 * nz * dz, 0, 0, 0]])
+    assert np.allclose(Vp, oracle.potential(nx, ny, nz, dx, (PERIODIC,) * 3, shifted, -1e9, 0.0, dy=dy, dz=dz), rtol=1e-12)
+    R0, J0 = oracle.wavepacket(nx, ny, nz, dx, 1.5, 1.0, 3.0, 0.9, 0.3, -0.4, 1.1, 2.0, dy=dy, dz=dz)
+    G = 2.0 * np.exp(-((i * dx - 1.5) ** 2 + (j * dy - 1.0) ** 2 + (k * dz - 3.0) ** 2) / (2 * 0.81))
+    phi = 0.3 * (i * dx - 1.5) - 0.4 * (j * dy - 1.0) + 1.1 * (k * dz - 3.0)
+    assert np.allclose(R0, G * np.cos(phi), atol=1e-14) and np.allclose(J0, G * np.sin(phi), atol=1e-14)

@@ -56,6 +56,8 @@ class Workload:
     every: int
     steps: int
     seeds: List[Optional[int]] = field(default_factory=list)
+    dy: Optional[float] = None      # None: cubic cells (dy = dz = dx); else the anisotropic mesh of PAPER.md:87, 142
+    dz: Optional[float] = None
 
     @property
     def cells(self) -> int:
