@@ -70,6 +70,13 @@ int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
 /* Free the context and everything the library allocated.  NULL is accepted. */
 int tdse_destroy(tdse_ctx* ctx);
 
+/* Anisotropic mesh (c_x, c_y, c_z = hbar dt / (2 m dx^2), ... ; the paper's own mesh is
+ * 35.4/240 x 40.9/240 x 70/420 Angstrom).  tdse_create makes cubic cells (dy = dz = dx); this call
+ * changes the spacing along y and z.  Grid point (i, j, k) sits at (i dx, j dy, k dz); the trace carries dx*dy, the
+ * norms dx*dy*dz.  Potential and state must be set again afterwards (TDSE_ESTATE from tdse_step otherwise).
+ * Errors: TDSE_EINVAL. */
+int tdse_set_spacing(tdse_ctx* ctx, double dy, double dz);
+
 /* Bytes of device workspace for the R, I, V grids (pingpong = 0: 3 arrays, two-pass kernels only;
  * pingpong = 1: 5 arrays, needed by the fused kernels).  Inside the workspace every xy plane is stored
  * with a frame of 4 columns and 4 rows on each side (periodic images or Dirichlet zeros, which lets the

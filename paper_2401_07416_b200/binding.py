@@ -30,7 +30,7 @@ SYMBOLS = [
     "tdse_set_wavepacket", "tdse_set_state", "tdse_set_detector", "tdse_step",
     "tdse_detector_read", "tdse_detector_device", "tdse_read_psi", "tdse_read_potential",
     "tdse_norm", "tdse_set_option", "tdse_get_info", "tdse_last_error",
-    "tdse_set_frames", "tdse_frames_read", "tdse_frames_device", "tdse_dissimilarity",
+    "tdse_set_frames", "tdse_frames_read", "tdse_frames_device", "tdse_dissimilarity", "tdse_set_spacing",
 ]
 
 
@@ -72,6 +72,7 @@ def load():
     L.tdse_step.argtypes = [vp, C.c_int]
     L.tdse_detector_read.argtypes = [vp, C.c_int, dp, dp, C.c_int, ip]
     L.tdse_detector_device.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), ip]
+    L.tdse_set_spacing.argtypes = [vp, C.c_double, C.c_double]
     L.tdse_set_frames.argtypes = [vp, C.c_int, C.c_int]
     L.tdse_frames_read.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, ip]
     L.tdse_frames_device.argtypes = [vp, C.POINTER(vp), ip, ip]
@@ -196,6 +197,9 @@ class Tdse:
         self._check(self.L.tdse_detector_device(self._h, C.byref(img), C.byref(tr), C.byref(ms)), "tdse_detector_device")
         return img.value, tr.value, ms.value
 
+    def set_spacing(self, dy, dz):
+        self._check(self.L.tdse_set_spacing(self._h, float(dy), float(dz)), "tdse_set_spacing")
+
     def set_frames(self, max_frames, include_t0=True):
         self._check(self.L.tdse_set_frames(self._h, int(max_frames), 1 if include_t0 else 0), "tdse_set_frames")
 
@@ -242,6 +246,8 @@ class Tdse:
     @classmethod
     def from_workload(cls, w, **kw) -> "Tdse":
         t = cls(w.nx, w.ny, w.nz, w.batch, w.dx, w.dt, w.mass, w.hbar, w.dtype, **kw)
+        if getattr(w, "dy", None) or getattr(w, "dz", None):
+            t.set_spacing(w.dy or w.dx, w.dz or w.dx)
         t.set_boundary(*w.bc, w.absorb_lo, w.absorb_hi, w.strength, w.power)
         for b in range(w.batch):
             t.set_potential(b, w.atoms[b], w.vmin, w.vmax, w.rcut)

@@ -35,7 +35,7 @@ struct tdse_ctx {
     int dtype = TDSE_F64;
     size_t w = 8;                       // bytes per element
     double dx = 0, dt = 0, mass = 0, hbar = 0;
-    double c = 0, cv = 0;
+    Mesh m{};                           // spacings (dx, dy, dz) and coefficients cx, cy, cz, c_v of PAPER.md:87
     int absorb_lo = 0, absorb_hi = 0, power = 2;
     double strength = 0.0;
 
@@ -349,7 +349,8 @@ int launch_fused_bc(tdse_ctx* c, FusedParams& P, int T)
 
 int launch_fused(tdse_ctx* c, FusedParams& P, int T)
 {
-    P.cf = (float)P.c; P.cvf = (float)P.cv; P.c6f = (float)(6.0 * P.c);
+    P.cxf = (float)P.cx; P.cyf = (float)P.cy; P.czf = (float)P.cz; P.cvf = (float)P.cv;
+    P.c2f = (float)(2.0 * (P.cx + P.cy + P.cz));
     P.entry_bytes = (unsigned long long)c->g.pcells * c->w;
     P.px = c->g.px; P.py = c->g.py;
     const bool ghostxy = c->g.bcx == BC_DIRICHLET || c->g.bcy == BC_DIRICHLET;
@@ -373,9 +374,9 @@ int launch_twopass_step(tdse_ctx* c)
     real* I = static_cast<real*>(c->I[c->cur]);
     const real* V = static_cast<const real*>(c->V);
     const real* M = static_cast<const real*>(c->mask_dev);
-    half_step_kernel<real><<<grid, 256, 0, c->stream>>>(c->g, (real)c->c, (real)c->cv, (real)1, V, M, R, I);
+    half_step_kernel<real><<<grid, 256, 0, c->stream>>>(c->g, (real)c->m.cx, (real)c->m.cy, (real)c->m.cz, (real)c->m.cv, (real)1, V, M, R, I);
     CU_LAUNCH_CHECK(c);
-    half_step_kernel<real><<<grid, 256, 0, c->stream>>>(c->g, (real)c->c, (real)c->cv, (real)-1, V, M, I, R);
+    half_step_kernel<real><<<grid, 256, 0, c->stream>>>(c->g, (real)c->m.cx, (real)c->m.cy, (real)c->m.cz, (real)c->m.cv, (real)-1, V, M, I, R);
     CU_LAUNCH_CHECK(c);
     return TDSE_OK;
 }
@@ -383,7 +384,7 @@ int launch_twopass_step(tdse_ctx* c)
 int finish_trace(tdse_ctx* c, int nparts)
 {
     trace_finish_kernel<<<(c->g.batch + 127) / 128, 128, 0, c->stream>>>(
-        c->partial, nparts, c->dx * c->dx, c->trace, c->max_samples, c->nsamples, c->g.batch);
+        c->partial, nparts, c->m.dx * c->m.dy, c->trace, c->max_samples, c->nsamples, c->g.batch);
     CU_LAUNCH_CHECK(c);
     c->nsamples++;
     return TDSE_OK;
@@ -458,8 +459,9 @@ int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
     c->g.pcells = c->g.pplane * nz;
     c->dtype = dtype; c->w = elem_bytes(dtype);
     c->dx = dx; c->dt = dt; c->mass = mass; c->hbar = hbar;
-    c->c = hbar * dt / (2.0 * mass * dx * dx);
-    c->cv = dt / hbar;
+    c->m.dx = c->m.dy = c->m.dz = dx;
+    c->m.cx = c->m.cy = c->m.cz = hbar * dt / (2.0 * mass * dx * dx);
+    c->m.cv = dt / hbar;
     c->arr_bytes = align_up((size_t)c->g.pcells * batch * c->w);
     c->have_V.assign(batch, 0);
     c->have_state.assign(batch, 0);
@@ -539,15 +541,29 @@ static int build_potential(tdse_ctx* c, int b, const AtomRec* atoms_dev, int nat
     const unsigned nblk = (unsigned)pot_bricks;
     void* dst = entry_ptr(c, c->V, b0);
     if (c->dtype == TDSE_F32)
-        potential_build_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->dx, atoms_dev, natoms, vmin, vmax, rcut, static_cast<float*>(dst));
+        potential_build_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, atoms_dev, natoms, vmin, vmax, rcut, static_cast<float*>(dst));
     else
-        potential_build_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->dx, atoms_dev, natoms, vmin, vmax, rcut, static_cast<double*>(dst));
+        potential_build_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, atoms_dev, natoms, vmin, vmax, rcut, static_cast<double*>(dst));
     CU_LAUNCH_CHECK(c);
     for (int e = b0 + 1; e < b1; ++e)
         CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->V, e), dst, (size_t)c->g.pcells * c->w, cudaMemcpyDeviceToDevice, c->stream));
     for (int e = b0; e < b1; ++e) c->have_V[e] = 1;
     c->vabs_max = std::max(c->vabs_max, std::max(std::fabs(vmin), std::fabs(vmax)));
     return TDSE_OK;
+}
+
+int tdse_set_spacing(tdse_ctx* c, double dy, double dz)
+{
+    if (!c) return TDSE_EINVAL;
+    if (!(dy > 0) || !(dz > 0)) return fail(c, TDSE_EINVAL, "tdse_set_spacing: dy, dz must be > 0");
+    c->m.dy = dy; c->m.dz = dz;
+    c->m.cy = c->hbar * c->dt / (2.0 * c->mass * dy * dy);
+    c->m.cz = c->hbar * c->dt / (2.0 * c->mass * dz * dz);
+    // potential and state were built on the old mesh
+    std::fill(c->have_V.begin(), c->have_V.end(), 0);
+    std::fill(c->have_state.begin(), c->have_state.end(), 0);
+    c->vabs_max = 0.0;
+    return reset_detector(c);
 }
 
 int tdse_set_potential(tdse_ctx* c, int b, const tdse_atom* atoms_host, int natoms, double vmin, double vmax, double rcut)
@@ -639,10 +655,10 @@ int tdse_set_wavepacket(tdse_ctx* c, int b, double x0, double y0, double z0, dou
     const unsigned nblk = (unsigned)((c->g.cells + 255) / 256);
     for (int e = b0; e < b1; ++e) {
         if (c->dtype == TDSE_F32)
-            wavepacket_init_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->dx, p, c->c, c->cv,
+            wavepacket_init_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->m, p,
                 (const float*)entry_ptr(c, c->V, e), (float*)entry_ptr(c, c->R[c->cur], e), (float*)entry_ptr(c, c->I[c->cur], e));
         else
-            wavepacket_init_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->dx, p, c->c, c->cv,
+            wavepacket_init_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->m, p,
                 (const double*)entry_ptr(c, c->V, e), (double*)entry_ptr(c, c->R[c->cur], e), (double*)entry_ptr(c, c->I[c->cur], e));
         CU_LAUNCH_CHECK(c);
         c->have_state[e] = 1;
@@ -690,7 +706,10 @@ int tdse_step(tdse_ctx* c, int n)
     for (int e = 0; e < c->g.batch; ++e)
         if (!c->have_V[e] || !c->have_state[e]) return fail(c, TDSE_ESTATE, "tdse_step: potential and state must be set for every entry");
     if (!c->allow_unstable) {
-        const double bound = 2.0 * c->hbar / (12.0 * c->hbar * c->hbar / (2.0 * c->mass * c->dx * c->dx) + c->vabs_max);
+        // largest eigenvalue of the discrete kinetic operator: (2 hbar^2 / m) (1/dx^2 + 1/dy^2 + 1/dz^2)
+        const double kin = 2.0 * c->hbar * c->hbar / c->mass *
+                           (1.0 / (c->m.dx * c->m.dx) + 1.0 / (c->m.dy * c->m.dy) + 1.0 / (c->m.dz * c->m.dz));
+        const double bound = 2.0 * c->hbar / (kin + c->vabs_max);
         if (c->dt > bound) {
             char buf[200];
             std::snprintf(buf, sizeof buf, "tdse_step: dt = %.6g exceeds the stability bound %.6g (max|V| = %.6g)", c->dt, bound, c->vabs_max);
@@ -729,7 +748,7 @@ int tdse_step(tdse_ctx* c, int n)
             P.mask = c->mask_dev;
             P.nx = c->g.nx; P.ny = c->g.ny; P.nz = c->g.nz; P.batch = c->g.batch;
             P.bcx = c->g.bcx; P.bcy = c->g.bcy; P.bcz = c->g.bcz;
-            P.c = c->c; P.cv = c->cv;
+            P.cx = c->m.cx; P.cy = c->m.cy; P.cz = c->m.cz; P.cv = c->m.cv;
             rc = launch_fused(c, P, T);
             if (rc) return rc;
             c->cur ^= 1;
@@ -814,7 +833,7 @@ int tdse_dissimilarity(tdse_ctx* c, int first_frame, int last_frame, double* d_h
     double* d_dev = c->partial + (size_t)batch * batch * nwin;
     const int tiles = (batch + kDisTile - 1) / kDisTile;
     dissimilarity_inner_kernel<<<dim3((unsigned)(tiles * tiles), (unsigned)nwin), 256, 0, c->stream>>>(
-        c->frames, batch, (long long)c->max_frames * c->g.plane, (int)c->g.plane, c->dx * c->dx, first_frame, nwin, inner);
+        c->frames, batch, (long long)c->max_frames * c->g.plane, (int)c->g.plane, c->m.dx * c->m.dy, first_frame, nwin, inner);
     CU_LAUNCH_CHECK(c);
     dissimilarity_finish_kernel<<<(batch * batch + 127) / 128, 128, 0, c->stream>>>(inner, batch, nwin, d_dev);
     CU_LAUNCH_CHECK(c);
@@ -864,13 +883,13 @@ int tdse_norm(tdse_ctx* c, int b, double* q_visscher, double* q_paper)
     int rc = ensure_partial(c, (size_t)2 * nblk);
     if (rc) return rc;
     if (c->dtype == TDSE_F32)
-        norm_partial_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->c, c->cv, (const float*)entry_ptr(c, c->V, b),
+        norm_partial_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->m, (const float*)entry_ptr(c, c->V, b),
             (const float*)c->mask_dev, (const float*)entry_ptr(c, c->R[c->cur], b), (const float*)entry_ptr(c, c->I[c->cur], b), c->partial);
     else
-        norm_partial_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->c, c->cv, (const double*)entry_ptr(c, c->V, b),
+        norm_partial_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->m, (const double*)entry_ptr(c, c->V, b),
             (const double*)c->mask_dev, (const double*)entry_ptr(c, c->R[c->cur], b), (const double*)entry_ptr(c, c->I[c->cur], b), c->partial);
     CU_LAUNCH_CHECK(c);
-    reduce_rows_kernel<<<1, 256, 0, c->stream>>>(c->partial, (int)nblk, 2, c->dx * c->dx * c->dx, c->scalars);
+    reduce_rows_kernel<<<1, 256, 0, c->stream>>>(c->partial, (int)nblk, 2, c->m.dx * c->m.dy * c->m.dz, c->scalars);
     CU_LAUNCH_CHECK(c);
     double q[2];
     CU_TRY(c, cudaMemcpyAsync(q, c->scalars, sizeof q, cudaMemcpyDeviceToHost, c->stream));

@@ -66,7 +66,7 @@ constexpr int kPotBX = 16, kPotBY = 4, kPotBZ = 4;
 
 template <typename real>
 __global__ void __launch_bounds__(256)
-potential_build_kernel(Grid g, double dx, const AtomRec* __restrict__ atoms, int natoms,
+potential_build_kernel(Grid g, double dx, double dy, double dz, const AtomRec* __restrict__ atoms, int natoms,
                        double vmin, double vmax, double rcut, real* __restrict__ V /* entry base */)
 {
     static_assert(kPotBX * kPotBY * kPotBZ == 256 && kAtomChunk <= 256, "block shape");
@@ -77,15 +77,15 @@ potential_build_kernel(Grid g, double dx, const AtomRec* __restrict__ atoms, int
     const int bx = blockIdx.x % bricks_x, by = (blockIdx.x / bricks_x) % bricks_y, bz = blockIdx.x / (bricks_x * bricks_y);
     const int i0 = (bx * kPotBX + tx) * kPotCells, j = by * kPotBY + ty, k = bz * kPotBZ + tz;
     const bool live = i0 < g.nx && j < g.ny && k < g.nz;
-    const double y = j * dx, z = k * dx;
-    const double Lx = g.nx * dx, Ly = g.ny * dx, Lz = g.nz * dx;
+    const double y = j * dy, z = k * dz;
+    const double Lx = g.nx * dx, Ly = g.ny * dy, Lz = g.nz * dz;
     const double iLx = 1.0 / Lx, iLy = 1.0 / Ly, iLz = 1.0 / Lz;
     const bool perx = g.bcx == BC_PERIODIC, pery = g.bcy == BC_PERIODIC, perz = g.bcz == BC_PERIODIC;
     const double rc2 = rcut * rcut;
     // the brick's bounding box, padded by a cell so that rounding never drops an atom the pair test would keep
     const double lox = (bx * kPotBX * kPotCells - 1) * dx, hix = ((bx + 1) * kPotBX * kPotCells) * dx;
-    const double loy = (by * kPotBY - 1) * dx, hiy = ((by + 1) * kPotBY) * dx;
-    const double loz = (bz * kPotBZ - 1) * dx, hiz = ((bz + 1) * kPotBZ) * dx;
+    const double loy = (by * kPotBY - 1) * dy, hiy = ((by + 1) * kPotBY) * dy;
+    const double loz = (bz * kPotBZ - 1) * dz, hiz = ((bz + 1) * kPotBZ) * dz;
     double sum[kPotCells];
 #pragma unroll
     for (int e = 0; e < kPotCells; ++e) sum[e] = 0.0;
@@ -153,11 +153,12 @@ potential_build_kernel(Grid g, double dx, const AtomRec* __restrict__ atoms, int
 // (wrapped) neighbour grid point, or are 0 beyond a Dirichlet face.
 // ---------------------------------------------------------------------------------------------
 struct PacketParams { double x0, y0, z0, inv2s2, kx, ky, kz, amp; };
+struct Mesh { double dx, dy, dz; double cx, cy, cz, cv; };   // spacings and the coefficients of PAPER.md:87
 
-__device__ __forceinline__ void packet_eval(const PacketParams& p, double dx, int i, int j, int k,
+__device__ __forceinline__ void packet_eval(const PacketParams& p, const Mesh& m, int i, int j, int k,
                                             double* re, double* im)
 {
-    const double ddx = i * dx - p.x0, ddy = j * dx - p.y0, ddz = k * dx - p.z0;
+    const double ddx = i * m.dx - p.x0, ddy = j * m.dy - p.y0, ddz = k * m.dz - p.z0;
     const double G = p.amp * exp(-(ddx * ddx + ddy * ddy + ddz * ddz) * p.inv2s2);
     const double phi = p.kx * ddx + p.ky * ddy + p.kz * ddz;
     double s, c;
@@ -166,20 +167,20 @@ __device__ __forceinline__ void packet_eval(const PacketParams& p, double dx, in
     *im = G * s;
 }
 
-__device__ __forceinline__ double packet_re_nbr(const PacketParams& p, const Grid& g, double dx,
+__device__ __forceinline__ double packet_re_nbr(const PacketParams& p, const Grid& g, const Mesh& m,
                                                 int i, int j, int k)
 {
     if (i < 0 || i >= g.nx) { if (g.bcx == BC_PERIODIC) i = wrap_index(i, g.nx); else return 0.0; }
     if (j < 0 || j >= g.ny) { if (g.bcy == BC_PERIODIC) j = wrap_index(j, g.ny); else return 0.0; }
     if (k < 0 || k >= g.nz) { if (g.bcz == BC_PERIODIC) k = wrap_index(k, g.nz); else return 0.0; }
     double re, im;
-    packet_eval(p, dx, i, j, k, &re, &im);
+    packet_eval(p, m, i, j, k, &re, &im);
     return re;
 }
 
 template <typename real>
 __global__ void __launch_bounds__(256)
-wavepacket_init_kernel(Grid g, double dx, PacketParams p, double c, double cv,
+wavepacket_init_kernel(Grid g, Mesh m, PacketParams p,
                        const real* __restrict__ V, real* __restrict__ R, real* __restrict__ I)
 {
     const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -189,11 +190,11 @@ wavepacket_init_kernel(Grid g, double dx, PacketParams p, double c, double cv,
     const int j = (int)(t % g.ny);
     const int k = (int)(t / g.ny);
     double re, im;
-    packet_eval(p, dx, i, j, k, &re, &im);
-    const double d2x = packet_re_nbr(p, g, dx, i + 1, j, k) - 2.0 * re + packet_re_nbr(p, g, dx, i - 1, j, k);
-    const double d2y = packet_re_nbr(p, g, dx, i, j + 1, k) - 2.0 * re + packet_re_nbr(p, g, dx, i, j - 1, k);
-    const double d2z = packet_re_nbr(p, g, dx, i, j, k + 1) - 2.0 * re + packet_re_nbr(p, g, dx, i, j, k - 1);
-    const double Ar = -c * d2x - c * d2y - c * d2z + cv * (double)V[cell_offset(g, i, j, k)] * re;
+    packet_eval(p, m, i, j, k, &re, &im);
+    const double d2x = packet_re_nbr(p, g, m, i + 1, j, k) - 2.0 * re + packet_re_nbr(p, g, m, i - 1, j, k);
+    const double d2y = packet_re_nbr(p, g, m, i, j + 1, k) - 2.0 * re + packet_re_nbr(p, g, m, i, j - 1, k);
+    const double d2z = packet_re_nbr(p, g, m, i, j, k + 1) - 2.0 * re + packet_re_nbr(p, g, m, i, j, k - 1);
+    const double Ar = -m.cx * d2x - m.cy * d2y - m.cz * d2z + m.cv * (double)V[cell_offset(g, i, j, k)] * re;
     store_with_images(R, g, i, j, k, (real)re);
     store_with_images(I, g, i, j, k, (real)(im + 0.5 * Ar));
 }
@@ -201,7 +202,7 @@ wavepacket_init_kernel(Grid g, double dx, PacketParams p, double c, double cv,
 // ---------------------------------------------------------------------------------------------
 // Two-pass reference stencil: one thread per cell, neighbours straight from global memory (L1/L2).
 //   sgn = +1: eq (9) PAPER.md:83  dst = I, src = R;   sgn = -1: eq (8) PAPER.md:74  dst = R, src = I
-//   dst <- M[k] * ( dst + sgn * ( c * (sum of 6 neighbours - 6 src) - c_v V src ) )
+//   dst <- M[k] * ( dst + sgn * ( c_x d2x(src) + c_y d2y(src) + c_z d2z(src) - c_v V src ) )
 // In place is safe (dst is read only at the thread's own cell).  Works for every shape and boundary
 // combination; the fused kernels in tdse_kernels_fused.cuh are the fast path.
 // ---------------------------------------------------------------------------------------------
@@ -219,7 +220,7 @@ __device__ __forceinline__ real load_nbr(const real* __restrict__ f, const Grid&
 
 template <typename real>
 __global__ void __launch_bounds__(256)
-half_step_kernel(Grid g, real c, real cv, real sgn, const real* __restrict__ V,
+half_step_kernel(Grid g, real cx, real cy, real cz, real cv, real sgn, const real* __restrict__ V,
                  const real* __restrict__ M, const real* __restrict__ src, real* __restrict__ dst)
 {
     // grid: x = cells of one entry / 256, y = batch entry
@@ -233,11 +234,10 @@ half_step_kernel(Grid g, real c, real cv, real sgn, const real* __restrict__ V,
     const real* s = src + base;
     const long long o = cell_offset(g, i, j, k);
     const real s0 = s[o];
-    const real nb = (load_nbr(s, g, i + 1, j, k) + load_nbr(s, g, i - 1, j, k))
-                  + (load_nbr(s, g, i, j + 1, k) + load_nbr(s, g, i, j - 1, k))
-                  + (load_nbr(s, g, i, j, k + 1) + load_nbr(s, g, i, j, k - 1));
-    const real lap = nb - (real)6 * s0;
-    const real upd = c * lap - cv * V[base + o] * s0;
+    const real d2x = (load_nbr(s, g, i + 1, j, k) + load_nbr(s, g, i - 1, j, k)) - (real)2 * s0;
+    const real d2y = (load_nbr(s, g, i, j + 1, k) + load_nbr(s, g, i, j - 1, k)) - (real)2 * s0;
+    const real d2z = (load_nbr(s, g, i, j, k + 1) + load_nbr(s, g, i, j, k - 1)) - (real)2 * s0;
+    const real upd = cx * d2x + cy * d2y + cz * d2z - cv * V[base + o] * s0;
     store_with_images(dst + base, g, i, j, k, M[k] * (dst[base + o] + sgn * upd));
 }
 
@@ -350,7 +350,7 @@ __global__ void trace_finish_kernel(const double* __restrict__ partial, int npar
 // ---------------------------------------------------------------------------------------------
 template <typename real>
 __global__ void __launch_bounds__(256)
-norm_partial_kernel(Grid g, double c, double cv, const real* __restrict__ V, const real* __restrict__ M,
+norm_partial_kernel(Grid g, Mesh m, const real* __restrict__ V, const real* __restrict__ M,
                     const real* __restrict__ R, const real* __restrict__ I, double* __restrict__ partial)
 {
     __shared__ double scratch[32];
@@ -363,10 +363,10 @@ norm_partial_kernel(Grid g, double c, double cv, const real* __restrict__ V, con
         const int k = (int)(t / g.ny);
         const long long o = cell_offset(g, i, j, k);
         const double r0 = (double)R[o], i0 = (double)I[o];
-        const double nb = ((double)load_nbr(R, g, i + 1, j, k) + (double)load_nbr(R, g, i - 1, j, k))
-                        + ((double)load_nbr(R, g, i, j + 1, k) + (double)load_nbr(R, g, i, j - 1, k))
-                        + ((double)load_nbr(R, g, i, j, k + 1) + (double)load_nbr(R, g, i, j, k - 1));
-        const double ip = (double)M[k] * (i0 + c * (nb - 6.0 * r0) - cv * (double)V[o] * r0);
+        const double d2x = ((double)load_nbr(R, g, i + 1, j, k) + (double)load_nbr(R, g, i - 1, j, k)) - 2.0 * r0;
+        const double d2y = ((double)load_nbr(R, g, i, j + 1, k) + (double)load_nbr(R, g, i, j - 1, k)) - 2.0 * r0;
+        const double d2z = ((double)load_nbr(R, g, i, j, k + 1) + (double)load_nbr(R, g, i, j, k - 1)) - 2.0 * r0;
+        const double ip = (double)M[k] * (i0 + m.cx * d2x + m.cy * d2y + m.cz * d2z - m.cv * (double)V[o] * r0);
         qv = r0 * r0 + ip * i0;
         qp = r0 * r0 + i0 * i0;
     }

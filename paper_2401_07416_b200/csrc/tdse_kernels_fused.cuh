@@ -1,10 +1,10 @@
 // tdse_kernels_fused.cuh -- the fused, temporally blocked FDTD step for sm_100a.
 //
 // One launch advances every batch entry by T full time steps = 2T half-steps ("stages"):
-//   stage 2m+1: I^{n+m+1/2} = M[k] * ( I^{n+m-1/2} + c * lap(R^{n+m})     - (6c + c_v V) R^{n+m}     )   eq (9)
-//   stage 2m+2: R^{n+m+1}   = M[k] * ( R^{n+m}     - c * lap(I^{n+m+1/2}) + (6c + c_v V) I^{n+m+1/2} )   eq (8)
-// where lap(f) = sum of the 6 neighbours (the -6 f of the three second differences is folded into the
-// diagonal), boundary handling per eqs (13)-(14) PAPER.md:126-136 (periodic) or zero-Dirichlet, and the
+//   stage 2m+1: I^{n+m+1/2} = M[k] * ( I^{n+m-1/2} + lap_c(R^{n+m})     - (2(cx+cy+cz) + c_v V) R^{n+m}     )   eq (9)
+//   stage 2m+2: R^{n+m+1}   = M[k] * ( R^{n+m}     - lap_c(I^{n+m+1/2}) + (2(cx+cy+cz) + c_v V) I^{n+m+1/2} )   eq (8)
+// where lap_c(f) = cx (f_{i+1} + f_{i-1}) + cy (f_{j+1} + f_{j-1}) + cz (f_{k+1} + f_{k-1}) (the -2 f of each second
+// difference is folded into the diagonal), boundary handling per eqs (13)-(14) PAPER.md:126-136 (periodic) or zero-Dirichlet, and the
 // absorbing mask M[k] (eq (10) PAPER.md:89-94 as a polynomial mask) fused into the same pass.
 //
 // Design (differs from the paper's one-thread-per-point kernel, on purpose):
@@ -45,8 +45,8 @@ struct FusedParams {
     int bcx, bcy, bcz;
     int px, py;                                        // framed row length / rows per plane
     int tiles_x, tiles_y, nchunks, bz;                 // z chunk length (last chunk may be shorter)
-    double c, cv;
-    float cf, cvf, c6f;                                // the same, rounded once on the host for float contexts
+    double cx, cy, cz, cv;                             // PAPER.md:87 (one coefficient per axis)
+    float cxf, cyf, czf, cvf, c2f;                     // the same and 2(cx+cy+cz), rounded once on the host for float contexts
     unsigned long long entry_bytes;                    // px*py*nz*sizeof(real)
 };
 
@@ -162,10 +162,9 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
     const int Z0 = chunk * P.bz;
     const int bzc = min(P.bz, P.nz - Z0);
     const real* __restrict__ gM = static_cast<const real*>(P.mask);
-    real c, cv, c6;
-    if constexpr (std::is_same<real, float>::value) { c = P.cf; cv = P.cvf; c6 = P.c6f; }
-    else { c = P.c; cv = P.cv; c6 = 6.0 * P.c; }
-    const real negc = -c;
+    real cx, cy, cz, cv, c2;                        // c2 = 2 (cx + cy + cz): the diagonal of the three second differences
+    if constexpr (std::is_same<real, float>::value) { cx = P.cxf; cy = P.cyf; cz = P.czf; cv = P.cvf; c2 = P.c2f; }
+    else { cx = P.cx; cy = P.cy; cz = P.cz; cv = P.cv; c2 = 2.0 * (P.cx + P.cy + P.cz); }
 
     // ---- per-thread geometry, fixed for the whole march ---------------------------------------
     // Threads beyond the last slot repeat the last slot (a halo corner): same loads, same values, no stores.
@@ -215,15 +214,15 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
     // ---- TMA producer (thread 0): plane pz_next -> ring slot, two half-plane boxes per array ---------
     int pz_next = Z0 - H;                            // next plane to stage (wrapped when z is periodic)
     if (P.bcz == BC_PERIODIC) pz_next = wrap_index(pz_next, P.nz);
-    const int cx = X0 - HX + PADX, cyp = (Y0 - H + PADY) / 2;   // box origin: x, row pair (Y0-H+PADY is even)
+    const int box_x = X0 - HX + PADX, box_yp = (Y0 - H + PADY) / 2;   // box origin: x, row pair (Y0-H+PADY is even)
     auto issue_plane = [&](int ring_off, int slot_idx) {
         // a Dirichlet ghost plane has an out-of-range z coordinate: the TMA unit fills the box with zeros
         unsigned long long* bar = full + slot_idx;
         mbar_expect_tx(bar, 3u * Tr::BOX_BYTES);
         real* dst = ringR + ring_off;
-        tma_load_5d(dst, &tmR, bar, cx, cyp, 0, pz_next, b);
-        tma_load_5d(dst + RD * PS, &tmI, bar, cx, cyp, 0, pz_next, b);
-        tma_load_5d(dst + 2 * RD * PS, &tmV, bar, cx, cyp, 0, pz_next, b);
+        tma_load_5d(dst, &tmR, bar, box_x, box_yp, 0, pz_next, b);
+        tma_load_5d(dst + RD * PS, &tmI, bar, box_x, box_yp, 0, pz_next, b);
+        tma_load_5d(dst + 2 * RD * PS, &tmV, bar, box_x, box_yp, 0, pz_next, b);
         ++pz_next;
         if (P.bcz == BC_PERIODIC && pz_next == P.nz) pz_next = 0;
     };
@@ -317,7 +316,7 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
             iold[j] = *reinterpret_cast<const V4*>(ringI + ro_prev + soff + j * HP);
             const V4 vraw = *reinterpret_cast<const V4*>(ringV + ro_prev + soff + j * HP);
 #pragma unroll
-            for (int e = 0; e < VW; ++e) nw.dg[j].e[e] = fma(cv, vraw.e[e], c6);
+            for (int e = 0; e < VW; ++e) nw.dg[j].e[e] = fma(cv, vraw.e[e], c2);
         }
 
 #pragma unroll
@@ -348,10 +347,11 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
                 for (int e = 0; e < VW; ++e) {
                     const real left = (e == 0) ? xm : ctr.e[e - 1];
                     const real right = (e == VW - 1) ? xp : ctr.e[e + 1];
-                    const real nb = ((left + right) + (ylo.e[e] + yhi.e[e])) + (zlo.e[e] + zhi.e[e]);
-                    // odd stages: older + (c nb - dg ctr); even stages: older - (c nb - dg ctr)
-                    const real u = (s & 1) ? fma(-dg.e[e], ctr.e[e], fma(c, nb, older.e[e]))
-                                           : fma(dg.e[e], ctr.e[e], fma(negc, nb, older.e[e]));
+                    const real xs = left + right, ys = ylo.e[e] + yhi.e[e], zs = zlo.e[e] + zhi.e[e];
+                    // odd stages: older + (cx xs + cy ys + cz zs - dg ctr); even stages: older - (...).  zs (which needs
+                    // this iteration's output of the previous stage) enters the chain last.
+                    const real u = (s & 1) ? fma(cz, zs, fma(-dg.e[e], ctr.e[e], fma(cy, ys, fma(cx, xs, older.e[e]))))
+                                           : fma(-cz, zs, fma(dg.e[e], ctr.e[e], fma(-cy, ys, fma(-cx, xs, older.e[e]))));
                     out[j].e[e] = m * u;
                 }
             }

@@ -291,6 +291,44 @@ def test_frames_and_dissimilarity_match_oracle(dtype, include_t0):
 
 
 # ------------------------------------------------------------------------------------------
+# anisotropic mesh (c_x != c_y != c_z)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel,tblock", VARIANTS)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_anisotropic_mesh_matches_oracle(kernel, tblock, dtype):
+    # the paper's mesh ratios: 35.4/240 : 40.9/240 : 70/420 Angstrom, here in bohr-sized numbers
+    w = make_config(1, n=(40, 36, 48), steps=37, dtype=dtype)
+    w = w.with_(dy=w.dx * 40.9 / 35.4, dz=w.dx * (70.0 / 420.0) / (35.4 / 240.0), every=6)
+    from paper_2401_07416_b200 import Tdse
+    t = Tdse.from_workload(w)
+    t.set_option("kernel", kernel)
+    t.set_option("tblock", tblock)
+    o = OracleRun.from_workload(w, entry=0, dtype="f64", round_to="f32" if dtype == "f32" else None)
+    assert o.dy == w.dy and o.dz == w.dz and len({o.coef[0], o.coef[1], o.coef[2]}) == 3
+    # S0 / S1 on the anisotropic mesh
+    V = t.read_potential(0)
+    R, I = t.read_psi(0)
+    if dtype == "f64":
+        assert np.max(np.abs(V - o.V64)) <= 1e-13 * max(1.0, np.max(np.abs(o.V64)))
+        assert rel_l2(R, o.R) < 1e-14 and rel_l2(I, o.I) < 1e-14
+    else:
+        assert np.all(np.abs(V.astype(np.float64) - o.V) <= np.spacing(np.abs(o.V).astype(np.float32)).astype(np.float64))
+        assert rel_l2(R, o.R) < 1e-7 and rel_l2(I, o.I) < 1e-7
+    t.step(w.steps)
+    o.step(w.steps)
+    assert t.get_info("kernel") == kernel
+    tol = TOL[dtype]
+    R, I = t.read_psi(0)
+    D, tr = t.detector_read(0)
+    assert rel_l2(R, o.R) < tol and rel_l2(I, o.I) < tol
+    assert rel_l2(D, o.D) < tol and rel_l2(tr, o.trace) < tol          # trace carries dx*dy
+    qv, qp = t.norm(0)
+    ov, op = o.norm()
+    assert abs(qv - ov) < 10 * tol * abs(ov) and abs(qp - op) < 10 * tol * abs(op)   # norms carry dx*dy*dz
+    t.close()
+
+
+# ------------------------------------------------------------------------------------------
 # edge cases and error behaviour of the boundary
 # ------------------------------------------------------------------------------------------
 def test_call_order_and_stability_errors():
