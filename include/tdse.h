@@ -115,6 +115,16 @@ int tdse_set_potential(tdse_ctx* ctx, int b, const tdse_atom* atoms_host, int na
 int tdse_set_potential_device(tdse_ctx* ctx, int b, const tdse_atom* atoms_device, int natoms,
                               double vmin, double vmax, double rcut);
 
+/* Potential from a unit-cell grid (PAPER.md:148, 213 step (ii): "expansion and interpolation of the electrostatic
+ * potential onto the mesh points"; the paper spends 15 min per configuration on the host here).  cell: mz*my*mx
+ * doubles, [z][y][x], HOST (on_device = 0) or DEVICE (on_device = 1), samples at spacings (ax/mx, ay/my,
+ * az/(mz-1)).  The cell repeats periodically in x and y (the slab's supercell); below z0 and above z0 + az the
+ * nearest z plane is used.  V at mesh point (i dx, j dy, k dz) is the trilinear interpolation at
+ * (i dx - x0, j dy - y0, k dz - z0), clamped to [vmin, vmax], rounded once to the context dtype (DESIGN.md
+ * reading 24).  b = -1: all entries.  The stability check uses max(|vmin|, |vmax|).  Errors: TDSE_EINVAL, TDSE_ECUDA. */
+int tdse_set_potential_cell(tdse_ctx* ctx, int b, const double* cell, int on_device, int mx, int my, int mz,
+                            double ax, double ay, double az, double x0, double y0, double z0, double vmin, double vmax);
+
 /* Raw potential grid for entry b (b = -1: the same grid for all entries), nx*ny*nz values of the
  * context dtype, layout [z][y][x]; on_device says where V lives (a gridded V). */
 int tdse_set_potential_grid(tdse_ctx* ctx, int b, const void* V, int on_device);

@@ -7,8 +7,8 @@ that file with gcc and marshals numpy arrays through ctypes.
 """
 from .driver import (build, lib, OracleRun, potential, mask, wavepacket, stagger,
                      coefficients, max_threads, set_threads, paper_time_step, paper_wavelength,
-                     dissimilarity)
+                     dissimilarity, potential_cell)
 
 __all__ = ["build", "lib", "OracleRun", "potential", "mask", "wavepacket", "stagger",
            "coefficients", "max_threads", "set_threads", "paper_time_step", "paper_wavelength",
-           "dissimilarity"]
+           "dissimilarity", "potential_cell"]

@@ -60,6 +60,7 @@ def lib():
                 h = getattr(L, "oracle_plane_density_" + sfx)
                 h.restype = None
                 h.argtypes = [C.c_int] * 3 + [rp, rp, dp]
+            L.oracle_potential_cell.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [dp] + [C.c_int] * 3 + [C.c_double] * 8 + [dp]
             L.oracle_dissimilarity.restype = C.c_double
             L.oracle_dissimilarity.argtypes = [dp, dp, C.c_int, C.c_double, C.c_int, C.c_int]
             _LIB = L
@@ -104,6 +105,19 @@ def potential(nx, ny, nz, dx, bc, atoms, vmin, vmax, rcut=0.0, dy=None, dz=None)
     dz = dx if dz is None else dz
     lib().oracle_potential(nx, ny, nz, dx, dy, dz, bc[0], bc[1], bc[2], _p(atoms, C.c_double),
                            atoms.shape[0], vmin, vmax, rcut, _p(V, C.c_double))
+    return V
+
+
+def potential_cell(nx, ny, nz, dx, cell, a, origin, vmin, vmax, dy=None, dz=None) -> np.ndarray:
+    """Unit-cell potential cell[mz][my][mx] of edge lengths a = (ax, ay, az), tiled in x, y and trilinearly
+    interpolated onto the mesh."""
+    cell = np.ascontiguousarray(cell, dtype=np.float64)
+    mz, my, mx = cell.shape
+    V = np.empty((nz, ny, nx), dtype=np.float64)
+    dy = dx if dy is None else dy
+    dz = dx if dz is None else dz
+    lib().oracle_potential_cell(nx, ny, nz, dx, dy, dz, _p(cell, C.c_double), mx, my, mz, a[0], a[1], a[2],
+                                origin[0], origin[1], origin[2], vmin, vmax, _p(V, C.c_double))
     return V
 
 
@@ -188,6 +202,11 @@ class OracleRun:
     # -- inputs ---------------------------------------------------------------------
     def set_potential_atoms(self, atoms, vmin, vmax, rcut=0.0):
         self.V64 = potential(self.nx, self.ny, self.nz, self.dx, self.bc, atoms, vmin, vmax, rcut, self.dy, self.dz)
+        self.V = self._round(self.V64)
+        return self
+
+    def set_potential_cell(self, cell, a, origin, vmin, vmax):
+        self.V64 = potential_cell(self.nx, self.ny, self.nz, self.dx, cell, a, origin, vmin, vmax, self.dy, self.dz)
         self.V = self._round(self.V64)
         return self
 

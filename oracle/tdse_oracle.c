@@ -19,6 +19,8 @@
  *   oracle_step_*      eqs (8), (9), (13), (14), (15): see tdse_oracle_step.inc.
  *   oracle_norm_*      PAPER.md:87 density and the conserved Visscher form.
  *   oracle_plane_density_*  one detector frame rho(i,j) = R^2 + I^2 on plane k_det (eq (15)).
+ *   oracle_potential_cell   unit-cell potential tiled in x, y and interpolated onto the mesh (
+ *                           DESIGN.md reading 24).
  *   oracle_dissimilarity    eq (16), between two frame trajectories (reading 23).
  *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): dense-eigh closed form on tiny grids, FFT
@@ -194,4 +196,45 @@ double oracle_dissimilarity(const double* rho_k, const double* rho_j, int npix, 
         acc += sqrt(dA * inner);
     }
     return acc / (double)(s1 - s0 + 1);
+}
+
+/* Potential from a unit-cell grid ("the values of the electrostatic potential at each grid point
+ * V(i,j,k) were obtained by interpolating the calculated potential"; PAPER.md:213 step (ii) "expansion and
+ * interpolation of the electrostatic potential onto the mesh points").  Reading: the unit cell
+ * holds cell[mz][my][mx] samples at spacings (ax/mx, ay/my, az/(mz-1)); it repeats periodically in x and y (the
+ * slab's supercell expansion) and is sampled by trilinear interpolation at the mesh point
+ * (i dx - x0, j dy - y0, k dz - z0); below z0 and above z0 + az the nearest z plane is used.  Then clamp. */
+void oracle_potential_cell(int nx, int ny, int nz, double dx, double dy, double dz,
+                           const double* cell, int mx, int my, int mz, double ax, double ay, double az,
+                           double x0, double y0, double z0, double vmin, double vmax, double* V)
+{
+    const double hx = ax / mx, hy = ay / my, hz = (mz > 1) ? az / (mz - 1) : 1.0;
+    for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double u = (i * dx - x0) / hx, v = (j * dy - y0) / hy, w = (k * dz - z0) / hz;
+                if (w < 0.0) w = 0.0;
+                if (w > (double)(mz - 1)) w = (double)(mz - 1);
+                const double fu = floor(u), fv = floor(v), fw = floor(w);
+                const double tu = u - fu, tv = v - fv;
+                int iw0 = (int)fw;
+                if (iw0 > mz - 2) iw0 = (mz > 1) ? mz - 2 : 0;
+                const double tw = (mz > 1) ? w - (double)iw0 : 0.0;
+                const int iw1 = (mz > 1) ? iw0 + 1 : 0;
+                long long iu0 = (long long)fu % mx; if (iu0 < 0) iu0 += mx;
+                long long iv0 = (long long)fv % my; if (iv0 < 0) iv0 += my;
+                const long long iu1 = (iu0 + 1) % mx, iv1 = (iv0 + 1) % my;
+#define CELL(a, b, c) cell[((size_t)(c) * my + (size_t)(b)) * mx + (size_t)(a)]
+                const double c00 = CELL(iu0, iv0, iw0) * (1.0 - tu) + CELL(iu1, iv0, iw0) * tu;
+                const double c10 = CELL(iu0, iv1, iw0) * (1.0 - tu) + CELL(iu1, iv1, iw0) * tu;
+                const double c01 = CELL(iu0, iv0, iw1) * (1.0 - tu) + CELL(iu1, iv0, iw1) * tu;
+                const double c11 = CELL(iu0, iv1, iw1) * (1.0 - tu) + CELL(iu1, iv1, iw1) * tu;
+#undef CELL
+                const double c0 = c00 * (1.0 - tv) + c10 * tv;
+                const double c1 = c01 * (1.0 - tv) + c11 * tv;
+                double val = c0 * (1.0 - tw) + c1 * tw;
+                if (val < vmin) val = vmin;
+                if (val > vmax) val = vmax;
+                V[((size_t)k * ny + j) * nx + i] = val;
+            }
 }

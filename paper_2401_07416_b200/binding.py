@@ -30,7 +30,7 @@ SYMBOLS = [
     "tdse_set_wavepacket", "tdse_set_state", "tdse_set_detector", "tdse_step",
     "tdse_detector_read", "tdse_detector_device", "tdse_read_psi", "tdse_read_potential",
     "tdse_norm", "tdse_set_option", "tdse_get_info", "tdse_last_error",
-    "tdse_set_frames", "tdse_frames_read", "tdse_frames_device", "tdse_dissimilarity", "tdse_set_spacing",
+    "tdse_set_frames", "tdse_frames_read", "tdse_frames_device", "tdse_dissimilarity", "tdse_set_spacing", "tdse_set_potential_cell",
 ]
 
 
@@ -73,6 +73,7 @@ def load():
     L.tdse_detector_read.argtypes = [vp, C.c_int, dp, dp, C.c_int, ip]
     L.tdse_detector_device.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), ip]
     L.tdse_set_spacing.argtypes = [vp, C.c_double, C.c_double]
+    L.tdse_set_potential_cell.argtypes = [vp, C.c_int, vp, C.c_int] + [C.c_int] * 3 + [C.c_double] * 8
     L.tdse_set_frames.argtypes = [vp, C.c_int, C.c_int]
     L.tdse_frames_read.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, ip]
     L.tdse_frames_device.argtypes = [vp, C.POINTER(vp), ip, ip]
@@ -153,6 +154,18 @@ class Tdse:
     def set_potential_device(self, b, atoms_tensor, natoms, vmin, vmax, rcut=0.0):
         self._check(self.L.tdse_set_potential_device(self._h, b, atoms_tensor.data_ptr(), natoms, vmin, vmax, rcut),
                     "tdse_set_potential_device")
+
+    def set_potential_cell(self, b, cell, a, origin, vmin, vmax):
+        if hasattr(cell, "data_ptr"):
+            mz, my, mx = cell.shape
+            ptr, dev = cell.data_ptr(), 1
+        else:
+            cell = np.ascontiguousarray(cell, dtype=np.float64)
+            mz, my, mx = cell.shape
+            ptr, dev = cell.ctypes.data, 0
+        self._check(self.L.tdse_set_potential_cell(self._h, b, ptr, dev, mx, my, mz, float(a[0]), float(a[1]), float(a[2]),
+                                                   float(origin[0]), float(origin[1]), float(origin[2]), vmin, vmax),
+                    "tdse_set_potential_cell")
 
     def set_potential_grid(self, b, V):
         if hasattr(V, "data_ptr"):

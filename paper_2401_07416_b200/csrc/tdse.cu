@@ -607,6 +607,44 @@ int tdse_set_potential_device(tdse_ctx* c, int b, const tdse_atom* atoms_device,
     return build_potential(c, b, reinterpret_cast<const AtomRec*>(atoms_device), natoms, vmin, vmax, rcut);
 }
 
+int tdse_set_potential_cell(tdse_ctx* c, int b, const double* cell, int on_device, int mx, int my, int mz,
+                            double ax, double ay, double az, double x0, double y0, double z0, double vmin, double vmax)
+{
+    if (!c) return TDSE_EINVAL;
+    if (!cell || mx < 1 || my < 1 || mz < 1) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: cell grid");
+    if (!(ax > 0) || !(ay > 0) || !(az > 0)) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: cell edge lengths must be > 0");
+    if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: vmin > vmax");
+    int b0, b1;
+    if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: entry out of range");
+    int rc = ensure_workspace(c);
+    if (rc) return rc;
+    const size_t n = (size_t)mx * my * mz;
+    const double* cell_dev = cell;
+    double* staged = nullptr;
+    if (!on_device) {
+        CU_TRY(c, cudaMalloc(&staged, n * sizeof(double)));
+        cudaError_t e = cudaMemcpyAsync(staged, cell, n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+        if (e != cudaSuccess) { cudaFree(staged); return fail(c, TDSE_ECUDA, std::string("tdse_set_potential_cell: ") + cudaGetErrorString(e)); }
+        cell_dev = staged;
+    }
+    CellParams p{mx, my, mz, ax, ay, az, x0, y0, z0, vmin, vmax};
+    const unsigned nblk = (unsigned)((c->g.cells + 255) / 256);
+    void* dst = entry_ptr(c, c->V, b0);
+    if (c->dtype == TDSE_F32)
+        potential_cell_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, cell_dev, p, static_cast<float*>(dst));
+    else
+        potential_cell_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, cell_dev, p, static_cast<double*>(dst));
+    cudaError_t le = cudaGetLastError();
+    if (staged) { cudaStreamSynchronize(c->stream); cudaFree(staged); }
+    if (le != cudaSuccess) return fail(c, TDSE_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(le));
+    c->launches++;
+    for (int e = b0 + 1; e < b1; ++e)
+        CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->V, e), dst, (size_t)c->g.pcells * c->w, cudaMemcpyDeviceToDevice, c->stream));
+    for (int e = b0; e < b1; ++e) c->have_V[e] = 1;
+    c->vabs_max = std::max(c->vabs_max, std::max(std::fabs(vmin), std::fabs(vmax)));
+    return TDSE_OK;
+}
+
 int tdse_set_potential_grid(tdse_ctx* c, int b, const void* V, int on_device)
 {
     if (!c) return TDSE_EINVAL;

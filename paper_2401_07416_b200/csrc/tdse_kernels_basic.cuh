@@ -147,6 +147,47 @@ potential_build_kernel(Grid g, double dx, double dy, double dz, const AtomRec* _
 }
 
 // ---------------------------------------------------------------------------------------------
+// Potential from a unit-cell grid (PAPER.md:148, 213 step (ii): expansion and interpolation of the DFT potential
+// onto the mesh; reading 24): cell[mz][my][mx] doubles at spacings (ax/mx, ay/my, az/(mz-1)), periodic
+// in x and y, nearest plane beyond the cell in z, trilinear interpolation at (i dx - x0, j dy - y0, k dz - z0),
+// clamp, one rounding to `real`.  One thread per cell; the gather hits L2 (a unit cell is small).
+// ---------------------------------------------------------------------------------------------
+struct CellParams { int mx, my, mz; double ax, ay, az, x0, y0, z0, vmin, vmax; };
+
+template <typename real>
+__global__ void __launch_bounds__(256)
+potential_cell_kernel(Grid g, double dx, double dy, double dz, const double* __restrict__ cell, CellParams p,
+                      real* __restrict__ V /* entry base */)
+{
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= g.cells) return;
+    const int i = (int)(c % g.nx);
+    const long long t = c / g.nx;
+    const int j = (int)(t % g.ny), k = (int)(t / g.ny);
+    const double hx = p.ax / p.mx, hy = p.ay / p.my, hz = (p.mz > 1) ? p.az / (p.mz - 1) : 1.0;
+    const double u = (i * dx - p.x0) / hx, v = (j * dy - p.y0) / hy;
+    const double w = fmin(fmax((k * dz - p.z0) / hz, 0.0), (double)(p.mz - 1));
+    const double fu = floor(u), fv = floor(v);
+    const double tu = u - fu, tv = v - fv;
+    int iw0 = min((int)floor(w), p.mz > 1 ? p.mz - 2 : 0);
+    const double tw = (p.mz > 1) ? w - (double)iw0 : 0.0;
+    const int iw1 = (p.mz > 1) ? iw0 + 1 : 0;
+    long long iu0 = (long long)fu % p.mx; if (iu0 < 0) iu0 += p.mx;
+    long long iv0 = (long long)fv % p.my; if (iv0 < 0) iv0 += p.my;
+    const long long iu1 = (iu0 + 1) % p.mx, iv1 = (iv0 + 1) % p.my;
+    auto at = [&](long long a, long long b, int cz) { return cell[((long long)cz * p.my + b) * p.mx + a]; };
+    // same grouping as the definition: x, then y, then z; products and sums kept separate (no contraction)
+    const double c00 = __dadd_rn(__dmul_rn(at(iu0, iv0, iw0), 1.0 - tu), __dmul_rn(at(iu1, iv0, iw0), tu));
+    const double c10 = __dadd_rn(__dmul_rn(at(iu0, iv1, iw0), 1.0 - tu), __dmul_rn(at(iu1, iv1, iw0), tu));
+    const double c01 = __dadd_rn(__dmul_rn(at(iu0, iv0, iw1), 1.0 - tu), __dmul_rn(at(iu1, iv0, iw1), tu));
+    const double c11 = __dadd_rn(__dmul_rn(at(iu0, iv1, iw1), 1.0 - tu), __dmul_rn(at(iu1, iv1, iw1), tu));
+    const double c0 = __dadd_rn(__dmul_rn(c00, 1.0 - tv), __dmul_rn(c10, tv));
+    const double c1 = __dadd_rn(__dmul_rn(c01, 1.0 - tv), __dmul_rn(c11, tv));
+    const double val = __dadd_rn(__dmul_rn(c0, 1.0 - tw), __dmul_rn(c1, tw));
+    store_with_images(V, g, i, j, k, (real)fmin(fmax(val, p.vmin), p.vmax));
+}
+
+// ---------------------------------------------------------------------------------------------
 // S1 packet init: eq (3) PAPER.md:52 with signed wave vector; staggered start
 //   R^0 = Re psi0,  I^{-1/2} = Im psi0 + (1/2) A Re psi0,  A f = -c d2 f + c_v V f   (reading 4)
 // evaluated in double from the stored V; neighbours of Re psi0 are re-evaluated analytically at the

@@ -329,6 +329,34 @@ def test_anisotropic_mesh_matches_oracle(kernel, tblock, dtype):
 
 
 # ------------------------------------------------------------------------------------------
+# unit-cell potential tiled and interpolated on the device
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_potential_cell_matches_oracle(dtype):
+    import torch
+    rng = np.random.default_rng(9)
+    cell = -5.0 * rng.random((9, 7, 6))
+    nx, ny, nz, dx, dy, dz = 44, 38, 30, 0.17, 0.21, 0.19
+    a, org = (1.9, 2.3, 4.0), (0.3, -0.7, 1.0)
+    t = make_ctx(nx, ny, nz, 2, dx, 0.001, dtype)
+    t.set_spacing(dy, dz)
+    t.set_boundary(PERIODIC, PERIODIC, DIRICHLET)
+    t.set_potential_cell(0, cell, a, org, -4.0, -0.5)                                    # host cell
+    t.set_potential_cell(1, torch.from_numpy(cell).cuda(), a, org, -4.0, -0.5)           # device cell
+    want = oracle.potential_cell(nx, ny, nz, dx, cell, a, org, -4.0, -0.5, dy, dz)
+    for b in range(2):
+        V = t.read_potential(b)
+        # the mesh coordinate i*dx - x0 may be fused into one FMA on the device: last-bit differences in the
+        # interpolation weights, continuous in the result
+        if dtype == "f64":
+            assert np.max(np.abs(V - want)) <= 1e-13 * np.max(np.abs(want))
+        else:
+            assert np.all(np.abs(V.astype(np.float64) - want) <= np.spacing(np.abs(want).astype(np.float32)).astype(np.float64))
+    assert want.min() == -4.0 and want.max() == -0.5   # both clamps are exercised
+    t.close()
+
+
+# ------------------------------------------------------------------------------------------
 # edge cases and error behaviour of the boundary
 # ------------------------------------------------------------------------------------------
 def test_call_order_and_stability_errors():

@@ -553,3 +553,39 @@ def test_anisotropic_potential_and_packet_closed_forms():
     G = 2.0 * np.exp(-((i * dx - 1.5) ** 2 + (j * dy - 1.0) ** 2 + (k * dz - 3.0) ** 2) / (2 * 0.81))
     phi = 0.3 * (i * dx - 1.5) - 0.4 * (j * dy - 1.0) + 1.1 * (k * dz - 3.0)
     assert np.allclose(R0, G * np.cos(phi), atol=1e-14) and np.allclose(J0, G * np.sin(phi), atol=1e-14)
+
+
+# ---------------------------------------------------------------------------------------
+# unit-cell potential tiled and interpolated onto the mesh (reading 24)
+# ---------------------------------------------------------------------------------------
+def test_potential_cell_interpolation_closed_forms():
+    mx, my, mz, ax, ay, az = 6, 5, 7, 1.8, 2.0, 3.0
+    hx, hy, hz = ax / mx, ay / my, az / (mz - 1)
+    kk, jj, ii = np.meshgrid(np.arange(mz), np.arange(my), np.arange(mx), indexing="ij")
+    nx, ny, nz, dx, dy, dz = 20, 18, 16, 0.17, 0.23, 0.21
+    org = (0.05, -0.3, 0.4)
+    K, J, I = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    X, Y, Z = I * dx - org[0], J * dy - org[1], K * dz - org[2]
+    big = 1e30
+    # (a) a cell that is linear in z only is reproduced exactly, with the nearest plane beyond the cell
+    V = oracle.potential_cell(nx, ny, nz, dx, 2.0 + 0.5 * kk * hz, (ax, ay, az), org, -big, big, dy, dz)
+    assert np.allclose(V, 2.0 + 0.5 * np.clip(Z, 0.0, az), rtol=0, atol=1e-13)
+    # (b) a periodic function sampled on a fine cell: the error obeys the linear-interpolation bound h^2 max|f''|/8
+    #     per axis, and the result is exactly periodic in x, y
+    f = lambda x, y, z: np.cos(2 * np.pi * x / ax) * np.sin(2 * np.pi * y / ay) * (1.0 + 0.3 * z)
+    fine = 8
+    kk2, jj2, ii2 = np.meshgrid(np.arange(mz), np.arange(my * fine), np.arange(mx * fine), indexing="ij")
+    cell = f(ii2 * hx / fine, jj2 * hy / fine, kk2 * hz)
+    V = oracle.potential_cell(nx, ny, nz, dx, cell, (ax, ay, az), org, -big, big, dy, dz)
+    want = f(X, Y, np.clip(Z, 0.0, az))
+    h2 = max((hx / fine) ** 2 * (2 * np.pi / ax) ** 2, (hy / fine) ** 2 * (2 * np.pi / ay) ** 2) / 8.0 * 2.0
+    assert np.max(np.abs(V - want)) <= 1.3 * (1.0 + 0.3 * az) * h2      # interpolation error bound of linear interpolation
+    shifted = oracle.potential_cell(nx, ny, nz, dx, cell, (ax, ay, az), (org[0] + 3 * ax, org[1] - 2 * ay, org[2]), -big, big, dy, dz)
+    assert np.allclose(V, shifted, rtol=0, atol=1e-12)
+    # (c) at mesh points that coincide with cell nodes the node value comes back; a constant cell stays constant; clamp
+    Vn = oracle.potential_cell(mx * 2, my * 2, mz, hx, np.arange(mz * my * mx, dtype=float).reshape(mz, my, mx),
+                               (ax, ay, az), (0.0, 0.0, 0.0), -big, big, hy, hz)
+    assert np.allclose(Vn[:, :my, :mx], np.arange(mz * my * mx).reshape(mz, my, mx), atol=1e-9)
+    assert np.allclose(Vn[:, my:, mx:], Vn[:, :my, :mx], atol=1e-9)                      # the supercell repeats
+    Vc = oracle.potential_cell(nx, ny, nz, dx, np.full((mz, my, mx), -3.5), (ax, ay, az), org, -2.0, 0.0, dy, dz)
+    assert np.all(Vc == -2.0)
