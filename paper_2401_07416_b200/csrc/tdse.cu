@@ -303,7 +303,7 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
     const int max_bz = (int)((kMaxSmem - Tr::SMEM_FIXED) / sizeof(real)) - 2 * H - 2;   // mask table must fit
     int best_n = 0;
     double best_cost = std::numeric_limits<double>::max();
-    const int max_chunks = std::max(1, c->g.nz / std::max(4 * H, 8));
+    const int max_chunks = std::max(1, c->g.nz / 2);   // chunks of >= 2 planes; the cost model below weighs the halo planes
     for (int n = 1; n <= std::max(std::max(max_chunks, c->opt_chunks), (c->g.nz + max_bz - 1) / max_bz); ++n) {
         const int bz = (c->g.nz + n - 1) / n;
         if (bz > max_bz) continue;
