@@ -339,7 +339,7 @@ def main():
     achieved = alg_bytes_per_launch / avg_launch_s / 1e9
     kname = "fdtd_fused_T%d_%s" % (tblock, w.dtype) if kernel == 2 else "half_step_%s" % w.dtype
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic_from_profiles(kname + "_" + a.workload), "kernel": kname, "peak_source": peak_src,
+                "traffic": traffic_from_profiles("%s_%s_b%d" % (kname, a.workload, w.batch)), "kernel": kname, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes_per_launch, "avg_launch_ms": avg_launch_s * 1e3,
                 "step_loop_gcell_per_s": step_value,
                 "frac_of_8TBps_nominal": achieved / 8000.0}
