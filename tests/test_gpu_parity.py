@@ -240,6 +240,58 @@ def test_config4_reduced_grid_fp32_vs_fp64_detector_agreement():
 
 
 # ------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times (tile, z chunks, batch): a few steps,
+# compared element by element with the oracle on sampled entries
+# ------------------------------------------------------------------------------------------
+def test_config3_full_batch_full_grid_sampled_entries():
+    """64 x 128^3 f32: the bench workload; entries 0, 31, 63 against the oracle after 24 steps (2 detector samples),
+    and the launch shape is the one bench.py reports."""
+    w = make_config(3, steps=24)
+    assert (w.batch, w.nx, w.ny, w.nz, w.dtype) == (64, 128, 128, 128, "f32")
+    worst, info = _run_config(w, w.steps, entries=(0, 31, 63))
+    assert info == (FUSED, 2) and worst < 1e-4
+
+
+def test_config2_full_grid_few_steps():
+    w = make_config(2, steps=40)
+    assert (w.nx, w.ny, w.nz, w.dtype) == (256, 256, 512, "f32")
+    worst, info = _run_config(w, w.steps)
+    assert info == (FUSED, 2) and worst < 1e-4
+
+
+@pytest.mark.parametrize("dtype,n", [("f32", 512), ("f64", 384)])
+def test_config4_full_grids_seeded_state(dtype, n):
+    """512^3 f32 / 384^3 f64 with the cfg-4 boundary set-up, seeded potential and state (the atom-list build at this
+    size is covered at reduced size: on the CPU it alone would take minutes), 6 steps, every cell compared."""
+    nx = ny = nz = n
+    dx = 0.15
+    dt = 0.5 / (6.0 / dx ** 2 + 200.0)
+    t = make_ctx(nx, ny, nz, 1, dx, dt, dtype)
+    t.set_boundary(PERIODIC, PERIODIC, DIRICHLET, 16, 16, 0.05, 2)
+    t.set_detector(10, 3, 4)
+    V = random_potential(41, (nz, ny, nx), -200.0, 0.0)
+    R0, I0 = random_state(42, (nz, ny, nx))
+    t.set_potential_grid(0, V.astype(t.np_dtype))
+    t.set_state(0, R0.astype(t.np_dtype), I0.astype(t.np_dtype))
+    o = OracleRun(nx, ny, nz, dx, dt, bc=(PERIODIC, PERIODIC, DIRICHLET), absorb_lo=16, absorb_hi=16, strength=0.05,
+                  round_to="f32" if dtype == "f32" else None)
+    o.set_potential_grid(V).set_state(R0, I0).set_detector(10, 3)
+    del V, R0, I0
+    t.step(6)
+    o.step(6)
+    assert (t.get_info("kernel"), t.get_info("tblock")) == (FUSED, 1)      # 6 = 2 + 1 (sample) + 2 + 1 (sample)
+    R, I = t.read_psi(0)
+    tol = TOL[dtype]
+    assert rel_l2(R, o.R) < tol and rel_l2(I, o.I) < tol
+    # per-cell bound as well: no tile, chunk seam or frame image may be off while the norm hides it
+    scale = float(np.max(np.abs(o.R)))
+    assert np.max(np.abs(R.astype(np.float64) - o.R)) < (1e-9 if dtype == "f64" else 1e-3) * scale
+    D, tr = t.detector_read(0)
+    assert len(tr) == 2 and rel_l2(D, o.D) < tol and rel_l2(tr, o.trace) < tol
+    t.close()
+
+
+# ------------------------------------------------------------------------------------------
 # frame-mode detector (PAPER.md:158-162) and pairwise dissimilarity (eq 16, PAPER.md:219-221)
 # ------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
