@@ -343,6 +343,41 @@ def test_frames_and_dissimilarity_match_oracle(dtype, include_t0):
 
 
 # ------------------------------------------------------------------------------------------
+# the paper's own boundary set-up: periodic on all three axes with an absorbing layer at one z face only
+# ("100 planes appended below the cell")
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel,tblock", VARIANTS)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_fully_periodic_with_one_face_absorber(kernel, tblock, dtype):
+    nx, ny, nz = 40, 24, 36
+    dx, dt, steps, batch = 0.25, 0.004, 31, 2
+    t = make_ctx(nx, ny, nz, batch, dx, dt, dtype)
+    t.set_boundary(PERIODIC, PERIODIC, PERIODIC, 0, 9, 0.07, 2)
+    t.set_option("kernel", kernel)
+    t.set_option("tblock", tblock)
+    t.set_detector(nz - 2, 4, 8)                    # detector plane inside the layer, next to the periodic seam
+    ora = []
+    for b in range(batch):
+        V = random_potential(300 + b, (nz, ny, nx), -30.0, 5.0)
+        R0, I0 = random_state(400 + b, (nz, ny, nx))
+        t.set_potential_grid(b, V.astype(t.np_dtype))
+        t.set_state(b, R0.astype(t.np_dtype), I0.astype(t.np_dtype))
+        o = OracleRun(nx, ny, nz, dx, dt, bc=(PERIODIC,) * 3, absorb_lo=0, absorb_hi=9, strength=0.07,
+                      round_to="f32" if dtype == "f32" else None)
+        o.set_potential_grid(V).set_state(R0, I0).set_detector(nz - 2, 4)
+        ora.append(o.step(steps))
+    assert np.all(ora[0].M[: nz - 9] == 1.0) and ora[0].M[-1] < 1.0      # one face only
+    t.step(steps)
+    tol = TOL[dtype]
+    for b in range(batch):
+        R, I = t.read_psi(b)
+        D, tr = t.detector_read(b)
+        assert rel_l2(R, ora[b].R) < tol and rel_l2(I, ora[b].I) < tol
+        assert rel_l2(D, ora[b].D) < tol and rel_l2(tr, ora[b].trace) < tol
+    t.close()
+
+
+# ------------------------------------------------------------------------------------------
 # anisotropic mesh (c_x != c_y != c_z)
 # ------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("kernel,tblock", VARIANTS)
