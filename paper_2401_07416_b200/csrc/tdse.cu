@@ -73,7 +73,7 @@ struct tdse_ctx {
     double vabs_max = 0.0;
 
     // options / info
-    int opt_kernel = TDSE_KERNEL_AUTO, opt_tblock = 0, allow_unstable = 0, opt_pf = 0, opt_chunks = 0;
+    int opt_kernel = TDSE_KERNEL_AUTO, opt_tblock = 0, allow_unstable = 0, opt_pf = 0, opt_chunks = 0, opt_pdl = 1;
     long long launches = 0;
     int last_kernel = 0, last_tblock = 0, last_tile_x = 0, last_tile_y = 0, last_chunks = 0;
     int num_sms = 148;
@@ -323,8 +323,16 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
     int rc = get_tensor_maps(c, Tr::W, Tr::NP, &maps);
     if (rc) return rc;
     const int in = c->cur;                              // maps: R[0], I[0], V, R[1], I[1]
-    kern<<<(unsigned)grid, NT, smem, c->stream>>>(P, maps[in ? 3 : 0], maps[in ? 4 : 1], maps[2]);
-    CU_LAUNCH_CHECK(c);
+    // Programmatic dependent launch: the next launch's CTAs may become resident and run their shared-memory
+    // prologue while this one drains; the kernel orders every global access behind griddepcontrol.wait.
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3(NT); lc.dynamicSmemBytes = smem; lc.stream = c->stream;
+    cudaLaunchAttribute la[1];
+    la[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    la[0].val.programmaticStreamSerializationAllowed = c->opt_pdl ? 1 : 0;
+    lc.attrs = la; lc.numAttrs = 1;
+    CU_TRY(c, cudaLaunchKernelEx(&lc, kern, P, maps[in ? 3 : 0], maps[in ? 4 : 1], maps[2]));
+    c->launches++;
     c->last_tile_x = BX; c->last_tile_y = BY; c->last_chunks = P.nchunks;
     return TDSE_OK;
 }
@@ -953,6 +961,8 @@ int tdse_set_option(tdse_ctx* c, const char* key, long long value)
     } else if (k == "z_chunks") {
         if (value < 0) return fail(c, TDSE_EINVAL, "tdse_set_option: z_chunks must be >= 0");
         c->opt_chunks = (int)value;
+    } else if (k == "pdl") {
+        c->opt_pdl = value ? 1 : 0;
     } else if (k == "allow_unstable") {
         c->allow_unstable = value ? 1 : 0;
     } else {

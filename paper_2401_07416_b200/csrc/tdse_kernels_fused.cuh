@@ -260,6 +260,14 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
         for (int i = 0; i < RD; ++i) mbar_init(full + i, 1);
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+    }
+    // Programmatic dependent launch: everything above touched only shared memory, kernel parameters and the mask
+    // table (which no kernel writes).  The previous launch in the stream wrote the arrays this one reads and
+    // read the arrays this one writes, so every thread waits for it to complete before its first global
+    // access; only then may the launch after this one become resident (at most one launch runs ahead).
+    asm volatile("griddepcontrol.wait;\n" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
+    if (tid == 0) {
 #pragma unroll
         for (int t = 0; t < PF; ++t) if (t < niter) issue_plane(t * PS, t);
     }
