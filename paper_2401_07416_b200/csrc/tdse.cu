@@ -377,14 +377,22 @@ bool fused_supported(const tdse_ctx* c)
 template <typename real>
 int launch_twopass_step(tdse_ctx* c)
 {
-    const dim3 grid((unsigned)((c->g.cells + 255) / 256), (unsigned)c->g.batch);
+    // z segments: enough blocks to fill the machine a few times over, at least 8 planes per segment
+    const long long cols = (long long)((c->g.nx + 31) / 32) * ((c->g.ny + 7) / 8) * c->g.batch;
+    int nseg = (int)std::min<long long>(std::max(1, c->g.nz / 8), std::max<long long>(1, (8LL * c->num_sms + cols - 1) / cols));
+    nseg = (int)std::min<long long>(nseg, std::max<long long>(1, 65535 / c->g.batch));
+    const int zs = (c->g.nz + nseg - 1) / nseg;
+    nseg = (c->g.nz + zs - 1) / zs;
+    if ((long long)c->g.batch * nseg > 65535) return fail(c, TDSE_EINVAL, "two-pass launch: batch too large for one grid");
+    const dim3 grid((unsigned)((c->g.nx + 31) / 32), (unsigned)((c->g.ny + 7) / 8), (unsigned)(c->g.batch * nseg));
+    const dim3 block(32, 8);
     real* R = static_cast<real*>(c->R[c->cur]);
     real* I = static_cast<real*>(c->I[c->cur]);
     const real* V = static_cast<const real*>(c->V);
     const real* M = static_cast<const real*>(c->mask_dev);
-    half_step_kernel<real><<<grid, 256, 0, c->stream>>>(c->g, (real)c->m.cx, (real)c->m.cy, (real)c->m.cz, (real)c->m.cv, (real)1, V, M, R, I);
+    half_step_kernel<real><<<grid, block, 0, c->stream>>>(c->g, (real)c->m.cx, (real)c->m.cy, (real)c->m.cz, (real)c->m.cv, (real)1, zs, nseg, V, M, R, I);
     CU_LAUNCH_CHECK(c);
-    half_step_kernel<real><<<grid, 256, 0, c->stream>>>(c->g, (real)c->m.cx, (real)c->m.cy, (real)c->m.cz, (real)c->m.cv, (real)-1, V, M, I, R);
+    half_step_kernel<real><<<grid, block, 0, c->stream>>>(c->g, (real)c->m.cx, (real)c->m.cy, (real)c->m.cz, (real)c->m.cv, (real)-1, zs, nseg, V, M, I, R);
     CU_LAUNCH_CHECK(c);
     return TDSE_OK;
 }

@@ -259,27 +259,54 @@ __device__ __forceinline__ real load_nbr(const real* __restrict__ f, const Grid&
     return f[cell_offset(g, i, j, k)];
 }
 
+// Block (32, 8): thread (tx, ty) owns the column (i, j) = (32 bx + tx, 8 by + ty) of one entry and marches a z segment
+// of `zs` planes, keeping the z neighbours of the source field in registers.  Neighbour offsets follow eqs (13)-(14)
+// (wrap on a periodic axis, zero beyond a Dirichlet face) and are fixed per column, so the loop has no index
+// arithmetic; the storage frame is written (store_with_images) but not relied on: domains narrower than two frames take this path.
+// grid: x = ceil(nx / 32), y = ceil(ny / 8), z = batch * nseg.  In place: a cell's update reads only its own dst.
 template <typename real>
 __global__ void __launch_bounds__(256)
-half_step_kernel(Grid g, real cx, real cy, real cz, real cv, real sgn, const real* __restrict__ V,
+half_step_kernel(Grid g, real cx, real cy, real cz, real cv, real sgn, int zs, int nseg, const real* __restrict__ V,
                  const real* __restrict__ M, const real* __restrict__ src, real* __restrict__ dst)
 {
-    // grid: x = cells of one entry / 256, y = batch entry
-    const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (cell >= g.cells) return;
-    const long long base = (long long)blockIdx.y * g.pcells;
-    const int i = (int)(cell % g.nx);
-    const long long t = cell / g.nx;
-    const int j = (int)(t % g.ny);
-    const int k = (int)(t / g.ny);
-    const real* s = src + base;
-    const long long o = cell_offset(g, i, j, k);
-    const real s0 = s[o];
-    const real d2x = (load_nbr(s, g, i + 1, j, k) + load_nbr(s, g, i - 1, j, k)) - (real)2 * s0;
-    const real d2y = (load_nbr(s, g, i, j + 1, k) + load_nbr(s, g, i, j - 1, k)) - (real)2 * s0;
-    const real d2z = (load_nbr(s, g, i, j, k + 1) + load_nbr(s, g, i, j, k - 1)) - (real)2 * s0;
-    const real upd = cx * d2x + cy * d2y + cz * d2z - cv * V[base + o] * s0;
-    store_with_images(dst + base, g, i, j, k, M[k] * (dst[base + o] + sgn * upd));
+    const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y;
+    if (i >= g.nx || j >= g.ny) return;
+    const int b = blockIdx.z / nseg, seg = blockIdx.z % nseg;
+    const int k0 = seg * zs, k1 = min(k0 + zs, g.nz);
+    const long long base = (long long)b * g.pcells;
+    const real* __restrict__ s = src + base;
+    const real* __restrict__ v = V + base;
+    real* __restrict__ d = dst + base;
+    int ix = 0, jy = 0;                  // shifts of the periodic images this column also stores (0: none)
+    if (g.bcx == BC_PERIODIC) { if (i < PADX) ix = g.nx; else if (i >= g.nx - PADX) ix = -g.nx; }
+    if (g.bcy == BC_PERIODIC) { if (j < PADY) jy = g.ny * g.px; else if (j >= g.ny - PADY) jy = -g.ny * g.px; }
+    auto plane_value = [&](int k) -> real {        // source value of this column at plane k, any k in [-1, nz]
+        if (k < 0)     { if (g.bcz == BC_PERIODIC) k = g.nz - 1; else return (real)0; }
+        if (k >= g.nz) { if (g.bcz == BC_PERIODIC) k = 0;        else return (real)0; }
+        return s[cell_offset(g, i, j, k)];
+    };
+    // x/y neighbour offsets relative to the cell, and whether the neighbour exists (else: Dirichlet zero)
+    const bool vxl = i > 0 || g.bcx == BC_PERIODIC, vxh = i < g.nx - 1 || g.bcx == BC_PERIODIC;
+    const bool vyl = j > 0 || g.bcy == BC_PERIODIC, vyh = j < g.ny - 1 || g.bcy == BC_PERIODIC;
+    const int oxl = i > 0 ? -1 : g.nx - 1, oxh = i < g.nx - 1 ? 1 : 1 - g.nx;
+    const int oyl = (j > 0 ? -1 : g.ny - 1) * g.px, oyh = (j < g.ny - 1 ? 1 : 1 - g.ny) * g.px;
+    real zlo = plane_value(k0 - 1), s0 = plane_value(k0);
+    long long o = cell_offset(g, i, j, k0);
+    for (int k = k0; k < k1; ++k, o += g.pplane) {
+        const real zhi = plane_value(k + 1);
+        const real xh = vxh ? s[o + oxh] : (real)0, xl = vxl ? s[o + oxl] : (real)0;
+        const real yh = vyh ? s[o + oyh] : (real)0, yl = vyl ? s[o + oyl] : (real)0;
+        const real d2x = (xh + xl) - (real)2 * s0;
+        const real d2y = (yh + yl) - (real)2 * s0;
+        const real d2z = (zhi + zlo) - (real)2 * s0;
+        const real upd = cx * d2x + cy * d2y + cz * d2z - cv * v[o] * s0;
+        const real out = M[k] * (d[o] + sgn * upd);
+        d[o] = out;
+        if (ix) d[o + ix] = out;
+        if (jy) d[o + jy] = out;
+        if (ix && jy) d[o + ix + jy] = out;
+        zlo = s0; s0 = zhi;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------

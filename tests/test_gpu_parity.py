@@ -146,6 +146,32 @@ def test_step_counts_split_across_calls_and_odd_sampling_period(kernel, tblock):
     a.close(); b.close()
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_dependent_launch_overlap_changes_nothing(dtype):
+    """The fused kernel is launched with programmatic stream serialization (the next launch's CTAs become resident
+    while the previous one drains).  Many back-to-back launches on a grid of a few CTAs, with detector samples, reads and a
+    host-side mask change in between, must give bit-identical results with the overlap switched off, and match the oracle."""
+    w = make_config(1, n=(40, 32, 24), steps=0).with_(dtype=dtype)
+    from paper_2401_07416_b200 import Tdse
+    res = []
+    for pdl in (1, 0):
+        t = Tdse.from_workload(w)
+        t.set_option("kernel", FUSED); t.set_option("pdl", pdl)
+        t.set_detector(5, 4, 64)
+        t.step(121)                                   # 60 T=2 launches + T=1 tails around the samples
+        mid = t.read_psi(0)
+        t.step(2); t.step(1); t.step(36)
+        res.append((mid, t.read_psi(0), t.detector_read(0)))
+        t.close()
+    for x, y in zip(res[0], res[1]):
+        assert np.array_equal(x[0], y[0]) and np.array_equal(x[1], y[1])
+    o = OracleRun.from_workload(w, dtype="f64", round_to="f32" if dtype == "f32" else None)
+    o.set_detector(5, 4).step(160)
+    tol = TOL[dtype]
+    (R, I), (D, tr) = res[0][1], res[0][2]
+    assert rel_l2(R, o.R) < tol and rel_l2(I, o.I) < tol and rel_l2(D, o.D) < tol and rel_l2(tr, o.trace) < tol
+
+
 def test_identical_entries_give_bitwise_identical_results_at_any_batch_position():
     w = make_config(3, n=(64, 48, 40), batch=1, steps=0)
     from paper_2401_07416_b200 import Tdse
