@@ -205,6 +205,8 @@ int tdse_norm(tdse_ctx* ctx, int b, double* q_visscher, double* q_paper);
 /* Options: "kernel" (TDSE_KERNEL_*), "tblock" (full steps fused per pass, 0 = auto, 1..2),
  * "prefetch" (planes the fused kernel keeps in flight through TMA, 0 = deepest that fits, 1..4),
  * "z_chunks" (z chunks per tile column in the fused launch, 0 = chosen by the launcher),
+ * "pdl" (0/1, default 1: fused launches carry the programmatic-stream-serialization attribute, so the next
+ * launch becomes resident while the previous one drains; results are bit-identical either way),
  * "allow_unstable" (0/1).  Errors: TDSE_EINVAL for unknown keys or values. */
 int tdse_set_option(tdse_ctx* ctx, const char* key, long long value);
 
