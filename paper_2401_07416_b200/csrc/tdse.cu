@@ -57,6 +57,7 @@ struct tdse_ctx {
     double* D = nullptr;                // [batch][ny][nx]
     double* trace = nullptr;            // [batch][max_samples]
     double* partial = nullptr;          // scratch for reductions
+    unsigned* done = nullptr;           // detector kernel: blocks finished per entry (returns to 0 after every sample)
     size_t partial_n = 0;
     double* scalars = nullptr;          // 4 doubles
     AtomRec* atoms_dev = nullptr;
@@ -397,12 +398,21 @@ int launch_twopass_step(tdse_ctx* c)
     return TDSE_OK;
 }
 
-int finish_trace(tdse_ctx* c, int nparts)
+// one launch per sample (accumulate + trace), programmatically serialised behind the step kernel
+template <typename real>
+int launch_detector(tdse_ctx* c, double* D, double* partial, double* frame, int slot)
 {
-    trace_finish_kernel<<<(c->g.batch + 127) / 128, 128, 0, c->stream>>>(
-        c->partial, nparts, c->m.dx * c->m.dy, c->trace, c->max_samples, c->nsamples, c->g.batch);
-    CU_LAUNCH_CHECK(c);
-    c->nsamples++;
+    const unsigned nblk = (unsigned)((c->g.plane + 255) / 256);
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3(nblk, (unsigned)c->g.batch); lc.blockDim = dim3(256); lc.dynamicSmemBytes = 0; lc.stream = c->stream;
+    cudaLaunchAttribute la[1];
+    la[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    la[0].val.programmaticStreamSerializationAllowed = c->opt_pdl ? 1 : 0;
+    lc.attrs = la; lc.numAttrs = 1;
+    CU_TRY(c, cudaLaunchKernelEx(&lc, detector_accum_kernel<real>, c->g, c->k_det, static_cast<const real*>(c->R[c->cur]),
+                                 static_cast<const real*>(c->I[c->cur]), D, partial, frame, (long long)c->max_frames * c->g.plane,
+                                 c->done, c->m.dx * c->m.dy, c->trace, c->max_samples, slot));
+    c->launches++;
     return TDSE_OK;
 }
 
@@ -412,24 +422,24 @@ int sample_detector(tdse_ctx* c)
     const unsigned nblk = (unsigned)((c->g.plane + 255) / 256);
     int rc = ensure_partial(c, (size_t)nblk * c->g.batch);
     if (rc) return rc;
+    if (!c->done) {
+        CU_TRY(c, cudaMalloc(&c->done, (size_t)c->g.batch * sizeof(unsigned)));
+        CU_TRY(c, cudaMemsetAsync(c->done, 0, (size_t)c->g.batch * sizeof(unsigned), c->stream));
+    }
     double* frame = (c->frames && c->nframes < c->max_frames) ? c->frames + (size_t)c->nframes * c->g.plane : nullptr;
-    detector_accum_kernel<real><<<dim3(nblk, (unsigned)c->g.batch), 256, 0, c->stream>>>(
-        c->g, c->k_det, static_cast<const real*>(c->R[c->cur]), static_cast<const real*>(c->I[c->cur]), c->D, c->partial,
-        frame, (long long)c->max_frames * c->g.plane);
-    CU_LAUNCH_CHECK(c);
+    rc = launch_detector<real>(c, c->D, c->partial, frame, c->nsamples);
+    if (rc) return rc;
     if (c->frames) c->nframes++;
-    return finish_trace(c, (int)nblk);
+    c->nsamples++;
+    return TDSE_OK;
 }
 
 // frame mode: rho(0) from the state in memory before the first step
 template <typename real>
 int sample_initial_frame(tdse_ctx* c)
 {
-    const unsigned nblk = (unsigned)((c->g.plane + 255) / 256);
-    detector_accum_kernel<real><<<dim3(nblk, (unsigned)c->g.batch), 256, 0, c->stream>>>(
-        c->g, c->k_det, static_cast<const real*>(c->R[c->cur]), static_cast<const real*>(c->I[c->cur]), nullptr, nullptr,
-        c->frames, (long long)c->max_frames * c->g.plane);
-    CU_LAUNCH_CHECK(c);
+    const int rc = launch_detector<real>(c, nullptr, nullptr, c->frames, 0);
+    if (rc) return rc;
     c->nframes = 1;
     return TDSE_OK;
 }
@@ -510,6 +520,7 @@ int tdse_destroy(tdse_ctx* c)
     if (c->trace) cudaFree(c->trace);
     if (c->frames) cudaFree(c->frames);
     if (c->partial) cudaFree(c->partial);
+    if (c->done) cudaFree(c->done);
     if (c->scalars) cudaFree(c->scalars);
     if (c->atoms_dev) cudaFree(c->atoms_dev);
     if (c->atoms_pin) cudaFreeHost(c->atoms_pin);

@@ -310,18 +310,25 @@ half_step_kernel(Grid g, real cx, real cy, real cz, real cv, real sgn, int zs, i
 }
 
 // ---------------------------------------------------------------------------------------------
-// S5 detector (eq (15), density of PAPER.md:87): D += R^2 + I^2 on plane k_det,
-// per-block partial sums (double) -> trace_finish_kernel sums them in fixed order.  Frame mode (the
-// trajectory rho = {rho(0), rho(h dt), ...}) also keeps the sampled plane: frame[b][p] = rho.  D, partial and
-// frame may each be NULL (frame-only call for rho(0)).  grid: x = ceil(nx*ny / 256), y = batch.
+// S5 detector (eq (15), density of PAPER.md:87): D += R^2 + I^2 on plane k_det and
+// trace[b][slot] = scale * sum of the plane (scale = dx dy), in ONE launch per sample: warp-shuffle block sums go
+// to partial[b][block]; the block that finishes last for an entry (a counter per entry, reset for the next sample)
+// adds the partials serially in block order, so the sum does not depend on which block that was.  Frame mode
+// (the trajectory rho = {rho(0), rho(h dt), ...}) also keeps the sampled plane: frame[b][p] = rho.
+// D, partial and frame may each be NULL (frame-only call for rho(0)).  grid: x = ceil(nx*ny / 256), y = batch.
+// Launched with programmatic stream serialization behind the fused step kernel: nothing global is touched before
+// griddepcontrol.wait.
 // ---------------------------------------------------------------------------------------------
 template <typename real>
 __global__ void __launch_bounds__(256)
 detector_accum_kernel(Grid g, int k_det, const real* __restrict__ R, const real* __restrict__ I,
                       double* __restrict__ D, double* __restrict__ partial /* [batch][gridDim.x] */,
-                      double* __restrict__ frame /* this sample's frame of entry 0 */, long long frame_entry_stride)
+                      double* __restrict__ frame /* this sample's frame of entry 0 */, long long frame_entry_stride,
+                      unsigned* __restrict__ done /* [batch] */, double scale, double* __restrict__ trace,
+                      int max_samples, int slot)
 {
     __shared__ double scratch[32];
+    asm volatile("griddepcontrol.wait;\n" ::: "memory");
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     double rho = 0.0;
     if (p < g.plane) {
@@ -333,7 +340,19 @@ detector_accum_kernel(Grid g, int k_det, const real* __restrict__ R, const real*
     }
     if (partial) {
         const double s = block_sum(rho, scratch);
-        if (threadIdx.x == 0) partial[(long long)blockIdx.y * gridDim.x + blockIdx.x] = s;
+        if (threadIdx.x == 0) {
+            double* part = partial + (long long)blockIdx.y * gridDim.x;
+            part[blockIdx.x] = s;
+            __threadfence();                                  // the partial is visible before the count
+            const unsigned before = atomicAdd(done + blockIdx.y, 1u);
+            if (before == gridDim.x - 1) {                    // every block of this entry has published its partial
+                __threadfence();
+                double t = 0.0;
+                for (unsigned q = 0; q < gridDim.x; ++q) t += __ldcg(part + q);   // fixed order; L2, not a stale L1 line
+                if (slot < max_samples) trace[(long long)blockIdx.y * max_samples + slot] = scale * t;
+                done[blockIdx.y] = 0;                         // ready for the next sample (same stream: ordered)
+            }
+        }
     }
 }
 
@@ -399,17 +418,6 @@ __global__ void dissimilarity_finish_kernel(const double* __restrict__ inner, in
     const double v = (k == j) ? 0.0 : acc / (double)nwin;
     d[(long long)k * batch + j] = v;
     d[(long long)j * batch + k] = v;
-}
-
-// trace[b][slot] = scale * sum_{q < nparts} partial[b][q]  (serial, fixed order).  One thread per entry.
-__global__ void trace_finish_kernel(const double* __restrict__ partial, int nparts, double scale,
-                                    double* __restrict__ trace, int max_samples, int slot, int batch)
-{
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= batch) return;
-    double s = 0.0;
-    for (int q = 0; q < nparts; ++q) s += partial[(long long)b * nparts + q];
-    if (slot < max_samples) trace[(long long)b * max_samples + slot] = scale * s;
 }
 
 // ---------------------------------------------------------------------------------------------
