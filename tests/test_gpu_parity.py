@@ -385,6 +385,43 @@ def test_config4_full_grids_seeded_state(dtype, n):
     t.close()
 
 
+def test_flat_offsets_beyond_2_31_elements_per_array():
+    """Maximum sizes: 18 entries of 512^3 f32 make every array 2.49e9 stored elements (9.3 GiB), so the last entries sit
+    beyond element 2^31 and byte 2^33.  All entries get the same seeded state: entry 0 is compared with the oracle cell by
+    cell, entries 16 and 17 (both beyond 2^31 elements) must be bit-identical to it, and so must their detector outputs."""
+    import torch
+    from workloads import random_state, random_potential
+    n, batch = 512, 18
+    assert 15 * (n + 8) * (n + 8) * n < 2 ** 31 < 16 * (n + 8) * (n + 8) * n
+    dx = 0.15
+    dt = 0.5 / (6.0 / dx ** 2 + 200.0)
+    t = make_ctx(n, n, n, batch, dx, dt, "f32")
+    t.set_boundary(PERIODIC, PERIODIC, DIRICHLET, 16, 16, 0.05, 2)
+    t.set_detector(10, 3, 4)
+    V = random_potential(43, (n, n, n), -200.0, 0.0)
+    R0, I0 = random_state(44, (n, n, n))
+    dev = [torch.from_numpy(a.astype(np.float32)).cuda() for a in (V, R0, I0)]
+    t.set_potential_grid(-1, dev[0])
+    t.set_state(-1, dev[1], dev[2])
+    torch.cuda.synchronize()
+    del dev
+    o = OracleRun(n, n, n, dx, dt, bc=(PERIODIC, PERIODIC, DIRICHLET), absorb_lo=16, absorb_hi=16, strength=0.05,
+                  round_to="f32")
+    o.set_potential_grid(V).set_state(R0, I0).set_detector(10, 3)
+    del V, R0, I0
+    t.step(6)
+    o.step(6)
+    assert t.get_info("kernel") == FUSED
+    R, I = t.read_psi(0)
+    D, tr = t.detector_read(0)
+    assert rel_l2(R, o.R) < 1e-4 and rel_l2(I, o.I) < 1e-4 and rel_l2(D, o.D) < 1e-4 and rel_l2(tr, o.trace) < 1e-4
+    for b in (16, 17):
+        Rb, Ib = t.read_psi(b)
+        Db, trb = t.detector_read(b)
+        assert np.array_equal(Rb, R) and np.array_equal(Ib, I) and np.array_equal(Db, D) and np.array_equal(trb, tr)
+    t.close()
+
+
 # ------------------------------------------------------------------------------------------
 # frame-mode detector (PAPER.md:158-162) and pairwise dissimilarity (eq 16, PAPER.md:219-221)
 # ------------------------------------------------------------------------------------------
