@@ -122,6 +122,65 @@ def test_recurrence_matches_oracle_on_random_states(kernel, tblock, dtype, shape
     t.close()
 
 
+@pytest.mark.parametrize("seed", [101, 102, 103])
+def test_randomised_configurations_every_kernel_variant(seed):
+    """Seeded random draws of everything at once -- shape (fused-eligible or not), batch, boundary flags, absorber
+    widths, anisotropic spacing, step count split over two calls, sampling period, detector plane, and for the fused
+    kernel the z chunking, prefetch depth and dependent-launch overlap -- each run through the two-pass kernel and
+    the fused kernel with T = 1 and T = 2 and compared with the oracle."""
+    from paper_2401_07416_b200 import Tdse
+    rng = np.random.default_rng(seed)
+    for case in range(8):
+        dtype = "f64" if rng.random() < 0.5 else "f32"
+        vw = 2 if dtype == "f64" else 4
+        nx = int(rng.integers(2, 40)) * vw if rng.random() < 0.8 else int(rng.integers(3, 90))
+        ny = int(rng.integers(4, 60)) * 2 if rng.random() < 0.8 else int(rng.integers(3, 90))
+        nz = int(rng.integers(2, 70))
+        batch = int(rng.integers(1, 4))
+        bc = tuple(int(x) for x in rng.integers(0, 2, 3))
+        alo, ahi = int(rng.integers(0, max(1, nz // 3))), int(rng.integers(0, max(1, nz // 3)))
+        steps, every, k_det = int(rng.integers(1, 14)), int(rng.integers(1, 6)), int(rng.integers(0, nz))
+        dx = 0.2
+        dy, dz = dx * (1.0 + 0.3 * rng.random()), dx * (1.0 - 0.3 * rng.random())
+        dt = 0.4 / (2.0 * (1 / dx ** 2 + 1 / dy ** 2 + 1 / dz ** 2) + 50.0)
+        V = [random_potential(seed * 1000 + case * 10 + b, (nz, ny, nx), -50.0, 0.0) for b in range(batch)]
+        S = [random_state(seed * 2000 + case * 10 + b, (nz, ny, nx)) for b in range(batch)]
+        oracles = []
+        for b in range(batch):
+            o = OracleRun(nx, ny, nz, dx, dt, bc=bc, absorb_lo=alo, absorb_hi=ahi, strength=0.06, power=2,
+                          round_to="f32" if dtype == "f32" else None, dy=dy, dz=dz)
+            o.set_potential_grid(V[b]).set_state(*S[b]).set_detector(k_det, every)
+            oracles.append(o.step(steps))
+        variants = [(TWOPASS, 1, 1)]
+        if fused_eligible(nx, ny, dtype):
+            variants += [(FUSED, 1, 1), (FUSED, 2, 1), (FUSED, 2, 0)]
+        for kernel, T, pdl in variants:
+            t = Tdse(nx, ny, nz, batch, dx, dt, 1.0, 1.0, dtype)
+            t.set_spacing(dy, dz)
+            t.set_boundary(bc[0], bc[1], bc[2], alo, ahi, 0.06, 2)
+            for b in range(batch):
+                t.set_potential_grid(b, V[b].astype(t.np_dtype))
+                t.set_state(b, S[b][0].astype(t.np_dtype), S[b][1].astype(t.np_dtype))
+            t.set_detector(k_det, every, 32)
+            t.set_option("kernel", kernel); t.set_option("tblock", T); t.set_option("pdl", pdl)
+            if kernel == FUSED and rng.random() < 0.5:
+                t.set_option("z_chunks", int(rng.integers(1, 6)))
+            if kernel == FUSED and rng.random() < 0.5:
+                t.set_option("prefetch", int(rng.integers(1, 3)))
+            first = int(rng.integers(0, steps + 1))
+            t.step(first); t.step(steps - first)
+            what = (seed, case, dtype, (nx, ny, nz), batch, bc, (alo, ahi), steps, every, k_det, kernel, T, pdl)
+            for b in range(batch):
+                R, I = t.read_psi(b)
+                D, tr = t.detector_read(b)
+                o = oracles[b]
+                assert len(tr) == len(o.trace) == steps // every, what
+                assert rel_l2(R, o.R) < TOL[dtype] and rel_l2(I, o.I) < TOL[dtype], what
+                if len(tr):
+                    assert rel_l2(D, o.D) < TOL[dtype] and rel_l2(tr, o.trace) < TOL[dtype], what
+            t.close()
+
+
 @pytest.mark.parametrize("kernel,tblock", VARIANTS)
 def test_step_counts_split_across_calls_and_odd_sampling_period(kernel, tblock):
     """n steps in one call == the same steps in uneven pieces; `every` odd forces T=1 launches in between."""
