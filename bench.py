@@ -153,6 +153,8 @@ def run_reference(a):
         return
     import oracle
     idx, w = workload_from_args(a)
+    # torchrun exports OMP_NUM_THREADS=1 to every rank; rank 0 alone runs this arm, on all the cores it may use
+    oracle.set_threads(len(os.sched_getaffinity(0)))
     cores = oracle.max_threads()
     nsample = 40 if w.cells <= 128 ** 3 else 4
     o = oracle.OracleRun.from_workload(w, entry=0, dtype=w.dtype)
