@@ -280,25 +280,16 @@ int get_tensor_maps(tdse_ctx* c, int W, int NP, const CUtensorMap** out)
     return TDSE_OK;
 }
 
-// ---------------------------------------------------------------------------------------------
-// fused launch table
-// ---------------------------------------------------------------------------------------------
-template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY, int MINB = 1>
-int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
+// z chunking of one fused variant: minimise waves * (chunk length + halo planes) on num_sms * ctas_per_sm slots.
+// Also used without launching, to compare variants (auto_tblock).  planes_out = planes one CTA marches times waves.
+template <typename real, int T, int BX, int BY, int NT, int PF, int MINB = 1>
+int plan_fused(tdse_ctx* c, int ctas_per_sm, int* tiles_x, int* tiles_y, int* bz_out, int* nchunks_out, long long* planes_out)
 {
     using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
-    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF, GHOSTXY, MINB>;
     constexpr size_t kMaxSmem = MINB == 1 ? 227 * 1024 : (228 * 1024) / MINB - 1024;   // per CTA (1 KB reserved each)
-    static_assert(Tr::SMEM_FIXED + 64 * sizeof(real) <= kMaxSmem, "fused tile does not fit in shared memory");
-    static bool attr_set = false;
-    if (!attr_set) {
-        CU_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
-        attr_set = true;
-    }
-    P.tiles_x = (c->g.nx + BX - 1) / BX;
-    P.tiles_y = (c->g.ny + BY - 1) / BY;
-    const long long units = (long long)P.tiles_x * P.tiles_y * c->g.batch;
-    // choose the number of z chunks: minimise waves * (chunk length + halo planes)
+    *tiles_x = (c->g.nx + BX - 1) / BX;
+    *tiles_y = (c->g.ny + BY - 1) / BY;
+    const long long units = (long long)*tiles_x * *tiles_y * c->g.batch;
     const long long slots = (long long)c->num_sms * ctas_per_sm;
     const int H = Tr::H;
     const int max_bz = (int)((kMaxSmem - Tr::SMEM_FIXED) / sizeof(real)) - 2 * H - 2;   // mask table must fit
@@ -315,13 +306,36 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
         if (cost < best_cost - 1e-9) { best_cost = cost; best_n = n_eff; }
     }
     if (best_n == 0) return fail(c, TDSE_EINVAL, "fused launch: no feasible z chunking");
-    P.bz = (c->g.nz + best_n - 1) / best_n;
-    P.nchunks = (c->g.nz + P.bz - 1) / P.bz;
+    *bz_out = (c->g.nz + best_n - 1) / best_n;
+    *nchunks_out = (c->g.nz + *bz_out - 1) / *bz_out;
+    if (planes_out) *planes_out = ((units * *nchunks_out + slots - 1) / slots) * (*bz_out + 2 * H);
+    return TDSE_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// fused launch table
+// ---------------------------------------------------------------------------------------------
+template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY, int MINB = 1>
+int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
+{
+    using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
+    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF, GHOSTXY, MINB>;
+    constexpr size_t kMaxSmem = MINB == 1 ? 227 * 1024 : (228 * 1024) / MINB - 1024;   // per CTA (1 KB reserved each)
+    static_assert(Tr::SMEM_FIXED + 64 * sizeof(real) <= kMaxSmem, "fused tile does not fit in shared memory");
+    static bool attr_set = false;
+    if (!attr_set) {
+        CU_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
+        attr_set = true;
+    }
+    int rc = plan_fused<real, T, BX, BY, NT, PF, MINB>(c, ctas_per_sm, &P.tiles_x, &P.tiles_y, &P.bz, &P.nchunks, nullptr);
+    if (rc) return rc;
+    const long long units = (long long)P.tiles_x * P.tiles_y * c->g.batch;
+    constexpr int H = Tr::H;
     const long long grid = units * P.nchunks;
     if (grid > 0x7fffffffLL) return fail(c, TDSE_EINVAL, "fused grid too large");
     const size_t smem = Tr::SMEM_FIXED + (size_t)(P.bz + 2 * H + 2) * sizeof(real);
     const CUtensorMap* maps = nullptr;
-    int rc = get_tensor_maps(c, Tr::W, Tr::NP, &maps);
+    rc = get_tensor_maps(c, Tr::W, Tr::NP, &maps);
     if (rc) return rc;
     const int in = c->cur;                              // maps: R[0], I[0], V, R[1], I[1]
     // Programmatic dependent launch: the next launch's CTAs may become resident and run their shared-memory
@@ -373,6 +387,28 @@ bool fused_supported(const tdse_ctx* c)
     // (also: even ny for the row-pair view, a domain at least as wide as the frame so that images are first images)
     return c->pingpong && (c->g.nx % vw == 0) && (c->g.ny % 2 == 0) && c->g.nx >= 2 * PADX && c->g.ny >= 2 * PADY &&
            ((unsigned long long)c->g.pcells * c->w < (1ull << 32));
+}
+
+// Temporal block when the caller leaves it open.  Two steps per pass halve the traffic but march 4 more halo planes
+// per chunk at 1.5x the time per plane; on grids so small that a chunk is a few planes (64^3) that costs more than
+// it saves.  Estimated time per step = (a_T + b_T * planes marched per CTA) / T with the constants measured on one
+// B200 (profiles/README.md, capture D: b = 0.77 / 1.16 us per plane for T = 1 / 2; a = 1.5 / 2.0 us with dependent
+// launch); T = 1 is taken only when it wins by 15 %, the accuracy of this model.
+int auto_tblock(tdse_ctx* c)
+{
+    int tx, ty, bz, nch;
+    long long p1 = 0, p2 = 0;
+    int rc1, rc2;
+    if (c->dtype == TDSE_F32) {
+        rc1 = plan_fused<float, 1, 64, 32, 352, 4>(c, 1, &tx, &ty, &bz, &nch, &p1);
+        rc2 = plan_fused<float, 2, 64, 32, 384, 2>(c, 1, &tx, &ty, &bz, &nch, &p2);
+    } else {
+        rc1 = plan_fused<double, 1, 32, 32, 352, 4>(c, 1, &tx, &ty, &bz, &nch, &p1);
+        rc2 = plan_fused<double, 2, 32, 24, 320, 3>(c, 1, &tx, &ty, &bz, &nch, &p2);
+    }
+    if (rc1 || rc2) return 2;
+    const double t1 = 1.5 + 0.77 * (double)p1, t2 = (2.0 + 1.16 * (double)p2) / 2.0;
+    return t1 < 0.85 * t2 ? 1 : 2;
 }
 
 template <typename real>
@@ -785,7 +821,7 @@ int tdse_step(tdse_ctx* c, int n)
     if (kernel == TDSE_KERNEL_AUTO) kernel = fused_supported(c) ? TDSE_KERNEL_FUSED : TDSE_KERNEL_TWOPASS;
     if (kernel == TDSE_KERNEL_FUSED && !fused_supported(c))
         return fail(c, TDSE_EINVAL, "tdse_step: fused kernel needs a 5-array workspace, rows of whole 16-byte groups, even ny, nx >= 8 and ny >= 8");
-    const int tmax = (c->opt_tblock > 0) ? c->opt_tblock : 2;
+    const int tmax = (c->opt_tblock > 0) ? c->opt_tblock : (kernel == TDSE_KERNEL_FUSED ? auto_tblock(c) : 1);
     c->last_kernel = kernel;
     if (n > 0 && c->frames && c->frames_t0 && c->every > 0 && c->steps == 0 && c->nframes == 0) {
         const int rc0 = (c->dtype == TDSE_F32) ? sample_initial_frame<float>(c) : sample_initial_frame<double>(c);

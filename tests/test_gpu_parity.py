@@ -289,7 +289,7 @@ def _run_config(w, steps, entries=None):
 def test_config0_full_size_full_steps():
     w = make_config(0)
     worst, info = _run_config(w, w.steps)
-    assert info == (FUSED, 2)
+    assert info == (FUSED, 1)       # 64^3: chunks of a few planes, the launcher's cost model takes one step per pass
     assert worst < 1e-11
 
 
