@@ -173,6 +173,59 @@ def test_visscher_norm_conserved_without_mask_and_decays_with_mask():
         last = q
 
 
+def mask_table(nz, w_lo, w_hi, strength, power):
+    """M[k] of DESIGN.md reading 6 (forward Euler on the quadratic CAP of eq (10)), written out here
+    independently of oracle.mask: xi = fractional depth into the layer, M = 1 - strength * xi^power."""
+    M = np.ones(nz)
+    for k in range(nz):
+        if w_lo > 0 and k < w_lo:
+            M[k] = 1.0 - strength * ((w_lo - k) / w_lo) ** power
+        if w_hi > 0 and k > nz - 1 - w_hi:
+            M[k] = 1.0 - strength * ((k - (nz - 1 - w_hi)) / w_hi) ** power
+    return M
+
+
+ABSORBER_CASES = [
+    # shape, bc, absorb_lo, absorb_hi, strength, power
+    ((4, 3, 8), (PERIODIC, PERIODIC, DIRICHLET), 3, 2, 0.30, 2),     # both z faces, different widths (cfg 1-4 layout)
+    ((3, 5, 7), (PERIODIC, PERIODIC, PERIODIC), 4, 0, 0.25, 2),      # the paper's own set-up: periodic z, one-face CAP
+    ((5, 2, 6), (DIRICHLET, PERIODIC, DIRICHLET), 0, 3, 0.40, 3),    # high face only, cubic profile
+    ((6, 6, 6), (DIRICHLET, DIRICHLET, PERIODIC), 2, 2, 0.20, 2),    # nx = ny = nz: an M[j]-for-M[k] slip still shows
+]
+
+
+@pytest.mark.parametrize("shape,bc,w_lo,w_hi,strength,power", ABSORBER_CASES)
+def test_absorber_inside_the_step_vs_dense_linear_map(shape, bc, w_lo, w_hi, strength, power):
+    """Where and how often the mask multiplies (readings 6-7; eq (10)).  One full step is
+    the linear map  I' = D_M (I - A R),  R' = D_M (R + A I'),  D_M = diag(M[k]) -- the mask acts on the freshly
+    updated field in BOTH half-steps, new = M (old + stencil).  Build that map densely with numpy from the
+    independent dense_A and mask_table, raise it to the n-th power, compare with the oracle stepping cell by cell.
+    A mask applied in one half-step only, M*old + stencil, or M indexed by the wrong axis each miss by > 1e-3."""
+    nx, ny, nz = shape
+    N = nx * ny * nz
+    dx, dt = 0.3, 0.01
+    V = random_potential(31, (nz, ny, nx), -3.0, 1.0)
+    R0, I0 = random_state(32, (nz, ny, nx))
+    n = 37
+    o = OracleRun(nx, ny, nz, dx, dt, bc=bc, absorb_lo=w_lo, absorb_hi=w_hi, strength=strength, power=power)
+    o.set_potential_grid(V).set_state(R0, I0).step(n)
+    c, _, _, cv = oracle.coefficients(dx, dt, 1.0, 1.0)
+    A = dense_A(nx, ny, nz, bc, c, cv, V)
+    DM = np.diag(np.repeat(mask_table(nz, w_lo, w_hi, strength, power), ny * nx))   # flat index (k*ny + j)*nx + i
+    E, Z = np.eye(N), np.zeros((N, N))
+    half_I = np.block([[E, Z], [-DM @ A, DM]])          # (R, I) -> (R, I')      eq (9) then mask
+    half_R = np.block([[DM, DM @ A], [Z, E]])           # (R, I') -> (R', I')    eq (8) then mask
+    S = np.linalg.matrix_power(half_R @ half_I, n)
+    want = S @ np.concatenate([R0.ravel(), I0.ravel()])
+    assert rel_l2(o.R, want[:N]) < 1e-12
+    assert rel_l2(o.I, want[N:]) < 1e-12
+    # the plausible mis-readings really are different maps on this input (so the bound above discriminates)
+    alt_one_half = np.linalg.matrix_power(half_R @ np.block([[E, Z], [-A, E]]), n)       # mask in eq (8) only
+    alt_old_only = np.linalg.matrix_power(np.block([[DM, A], [Z, E]]) @ np.block([[E, Z], [-A, DM]]), n)   # M*old + stencil
+    for alt in (alt_one_half, alt_old_only):
+        assert rel_l2((alt @ np.concatenate([R0.ravel(), I0.ravel()]))[:N], want[:N]) > 1e-3
+
+
 def test_stationary_eigenvector_has_constant_visscher_density():
     nx, ny, nz = 4, 3, 5
     bc = (DIRICHLET, PERIODIC, DIRICHLET)
