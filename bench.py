@@ -179,14 +179,36 @@ def run_reference(a):
 
 
 def cpu_baseline(w):
+    """The oracle as it stands on this box's host cores, bounded sample (~25 s): the parity build on all cores (the
+    headline `value`) and on one core, and the -O3 -march=native build of the same source."""
     import oracle
+    ncores = len(os.sched_getaffinity(0))
+    oracle.set_threads(ncores)
     cores = oracle.max_threads()
     o = oracle.OracleRun.from_workload(w, entry=0, dtype=w.dtype)
-    t0 = time.perf_counter(); o.step(4); probe = (time.perf_counter() - t0) / 4
-    n = int(max(4, min(w.steps, 12.0 / max(probe, 1e-6))))
-    t0 = time.perf_counter(); o.step(n); dt = time.perf_counter() - t0
-    return {"value": w.cells * n / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": "entry 0 of %s, %d of %d FDTD steps (%.1f s)" % (w.name, n, w.steps, dt)}
+
+    def timed(variant, threads, budget_s):
+        oracle.set_threads(threads, variant)
+        o.step_variant = variant
+        t0 = time.perf_counter(); o.step(2); probe = (time.perf_counter() - t0) / 2
+        n = int(max(2, min(w.steps, budget_s / max(probe, 1e-6))))
+        t0 = time.perf_counter(); o.step(n); dt = time.perf_counter() - t0
+        return w.cells * n / dt / 1e9, n, dt
+
+    v_all, n_all, dt_all = timed("parity", cores, 10.0)
+    v_one, n_one, _ = timed("parity", 1, 4.0)
+    v_fast, n_fast, _ = timed("timing", cores, 4.0)
+    v_fast1, n_fast1, _ = timed("timing", 1, 4.0)
+    oracle.set_threads(cores)
+    o.step_variant = "parity"
+    return {"value": v_all, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "entry 0 of %s, %d of %d FDTD steps (%.1f s), parity build (gcc -O2 -ffp-contract=off -fopenmp)" % (
+                w.name, n_all, w.steps, dt_all),
+            "serial": {"value": v_one, "cores": 1, "fdtd_steps": n_one, "ns_per_point_step": 1.0 / v_one},
+            "timing_build": {"flags": "gcc -O3 -march=native -fopenmp (same source; timing only, never parity)",
+                             "value": v_fast, "cores": cores, "fdtd_steps": n_fast,
+                             "serial_value": v_fast1, "serial_fdtd_steps": n_fast1,
+                             "serial_ns_per_point_step": 1.0 / v_fast1}}
 
 
 def fp32_vs_fp64_agreement(device):
@@ -237,15 +259,16 @@ def main():
     wbytes = 4 if w.dtype == "f32" else 8
 
     # device-resident inputs for `value`; pinned host inputs for `e2e`
-    atoms_dev = [torch.from_numpy(np.ascontiguousarray(x)).to("cuda:%d" % local_rank) for x in w.atoms]
-    atoms_host = [np.ascontiguousarray(x) for x in w.atoms]
+    # all entries' atom lists, concatenated (tdse_set_potential_batch: one launch builds every entry's V)
+    atoms_host = np.ascontiguousarray(np.concatenate(w.atoms, axis=0))
+    offsets = np.concatenate([[0], np.cumsum([x.shape[0] for x in w.atoms])]).astype(np.int32)
+    atoms_dev = torch.from_numpy(atoms_host).to("cuda:%d" % local_rank)
     img_host = torch.empty((w.batch, w.ny, w.nx), dtype=torch.float64).pin_memory().numpy()
     tr_host = np.zeros((w.batch, max_samples))
     torch.cuda.synchronize()
 
     def one_pass_device():
-        for b in range(w.batch):
-            t.set_potential_device(b, atoms_dev[b], w.atoms[b].shape[0], w.vmin, w.vmax, w.rcut)
+        t.set_potential_batch(atoms_dev, offsets, w.vmin, w.vmax, w.rcut)
         t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
         t.set_detector(w.k_det, w.every, max_samples)
         t.step(w.steps)
@@ -253,8 +276,7 @@ def main():
     import ctypes as C
 
     def one_pass_host():
-        for b in range(w.batch):
-            t.set_potential(b, atoms_host[b], w.vmin, w.vmax, w.rcut)
+        t.set_potential_batch(atoms_host, offsets, w.vmin, w.vmax, w.rcut)
         t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
         t.set_detector(w.k_det, w.every, max_samples)
         t.step(w.steps)
@@ -294,8 +316,7 @@ def main():
         ev[0].record(stream)
         for _ in range(a.steps):
             # S0, S1 then the step loop bracketed by its own events (dominant-kernel timing)
-            for b in range(w.batch):
-                t.set_potential_device(b, atoms_dev[b], w.atoms[b].shape[0], w.vmin, w.vmax, w.rcut)
+            t.set_potential_batch(atoms_dev, offsets, w.vmin, w.vmax, w.rcut)
             t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
             t.set_detector(w.k_det, w.every, max_samples)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -327,7 +348,7 @@ def main():
             one_pass_host()
         torch.cuda.synchronize()
         e2e_s = max_over_ranks(time.perf_counter() - t0)
-        h2d = sum(x.nbytes for x in atoms_host)
+        h2d = atoms_host.nbytes
         d2h = img_host.nbytes + tr_host.nbytes
         e2e = {"value": cell_updates / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e2e_s / a.steps}
@@ -340,9 +361,17 @@ def main():
     avg_launch_s = (step_ms * 1e-3) / max(nlaunch_step, 1)
     achieved = alg_bytes_per_launch / avg_launch_s / 1e9
     kname = "fdtd_fused_T%d_%s" % (tblock, w.dtype) if kernel == 2 else "half_step_%s" % w.dtype
+    # what DRAM moved per launch: the ncu capture of this kernel on this workload (profiles/roofline_traffic.csv), else
+    # the compulsory traffic of one launch on a flat layout (5 words per cell, whatever T; two-pass: 4 words per half-step)
+    traffic = traffic_from_profiles("%s_%s_b%d" % (kname, a.workload, w.batch))
+    compulsory = (5.0 if kernel == 2 else 4.0) * wbytes * float(w.cells) * w.batch
+    dram_bytes = traffic if traffic is not None else compulsory
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic_from_profiles("%s_%s_b%d" % (kname, a.workload, w.batch)), "kernel": kname, "peak_source": peak_src,
+                "traffic": traffic, "kernel": kname, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes_per_launch, "avg_launch_ms": avg_launch_s * 1e3,
+                "dram_gbs": dram_bytes / avg_launch_s / 1e9, "dram_frac": dram_bytes / avg_launch_s / 1e9 / peak,
+                "dram_bytes_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum (profiles/roofline_traffic.csv)"
+                                     if traffic is not None else "compulsory bytes per launch on a flat layout (no ncu capture of this workload)",
                 "step_loop_gcell_per_s": step_value,
                 "frac_of_8TBps_nominal": achieved / 8000.0}
 

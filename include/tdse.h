@@ -63,6 +63,9 @@ enum {
 /* Create a context for `batch` independent nx*ny*nz grids with cubic cells of edge dx, time step dt,
  * particle mass `mass`, reduced Planck constant `hbar`, arithmetic/storage type `dtype`.
  * Defaults: periodic on all three axes, no absorber, detector off.
+ * The context belongs to the CUDA device that is current in this call: every later call on it runs on that device
+ * whatever device the caller has current then (and leaves the caller's device current on return); a workspace
+ * passed to tdse_bind must live on it.
  * Errors: TDSE_EINVAL (sizes < 1, non-positive dx/dt/mass/hbar, unknown dtype), TDSE_ECUDA, TDSE_ENOMEM. */
 int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
                 double dx, double dt, double mass, double hbar, int dtype);
@@ -97,7 +100,9 @@ int tdse_bind(tdse_ctx* ctx, void* dev_workspace, size_t bytes, void* cuda_strea
  *   M[k] = 1 - strength * xi^power,  xi = (absorb_lo - k)/absorb_lo  for k < absorb_lo,
  *                                    xi = (k - (nz-1-absorb_hi))/absorb_hi  for k > nz-1-absorb_hi,
  * M = 1 elsewhere; 0 cells = that layer is off.  Errors: TDSE_EINVAL (unknown bc, negative widths,
- * absorb_lo + absorb_hi > nz, strength outside [0, 1], power < 1). */
+ * absorb_lo + absorb_hi > nz, strength outside [0, 1], power < 1).
+ * May be called before or after potential and state are loaded: when an x or y flag changes, the private storage
+ * frames (tdse_workspace_bytes) of the data already loaded are rewritten for the new flags. */
 int tdse_set_boundary(tdse_ctx* ctx, int bcx, int bcy, int bcz,
                       int absorb_lo, int absorb_hi, double strength, int power);
 
@@ -114,6 +119,18 @@ int tdse_set_potential(tdse_ctx* ctx, int b, const tdse_atom* atoms_host, int na
  * build kernel; the library does not copy it). */
 int tdse_set_potential_device(tdse_ctx* ctx, int b, const tdse_atom* atoms_device, int natoms,
                               double vmin, double vmax, double rcut);
+
+/* Build V for every entry in ONE launch (BASELINE.json north_star (4): many independent configurations, e.g. the
+ * paper's 879 thin-film structures): entry e uses atoms[offsets_host[e] .. offsets_host[e+1]) of one
+ * concatenated list.  `offsets_host` is a HOST array of batch+1 non-decreasing ints; `atoms` is in host memory
+ * (on_device = 0) or in device memory (on_device = 1, not copied: must stay valid until the stream reaches the build
+ * kernel).  Same definition and summation order as tdse_set_potential.  Atoms that every list starts with (a shared
+ * substrate) are found by the library (bitwise comparison) and summed once: a cell's sum then starts from the
+ * shared partial sum, which is the same sequence of operations as the plain list-order sum, so the result does not
+ * depend on it.  With on_device = 1 and batch >= 2 the call synchronises the stream once (one int comes back).
+ * Errors: TDSE_EINVAL (NULL, decreasing offsets, vmin > vmax), TDSE_ENOMEM, TDSE_ECUDA. */
+int tdse_set_potential_batch(tdse_ctx* ctx, const tdse_atom* atoms, const int* offsets_host, int on_device,
+                             double vmin, double vmax, double rcut);
 
 /* Potential from a unit-cell grid (PAPER.md:148, 213 step (ii): "expansion and interpolation of the electrostatic
  * potential onto the mesh points"; the paper spends 15 min per configuration on the host here).  cell: mz*my*mx
@@ -148,7 +165,9 @@ int tdse_set_state(tdse_ctx* ctx, int b, const void* R, const void* I_half, int 
  *   rho(i,j) = R^s(i,j,k)^2 + I^{s-1/2}(i,j,k)^2      (density of PAPER.md:87)
  * to a per-entry image (double) and appends dx^2 * sum_ij rho to a per-entry trace.  Resets image,
  * trace and step counter.  `max_samples` traces are kept per entry (further samples still accumulate
- * into the image but are not recorded in the trace).  Errors: TDSE_EINVAL. */
+ * into the image but are not recorded in the trace).  The trace buffer is kept (and its device pointer stays
+ * valid) while `max_samples` does not change; with the same `max_samples` the call does not synchronise.
+ * Errors: TDSE_EINVAL; TDSE_ENOMEM (the previous detector set-up is still in force). */
 int tdse_set_detector(tdse_ctx* ctx, int k_plane, int every, int max_samples);
 
 /* Advance every entry by n full time steps (eq (9) then eq (8), mask, detector), asynchronously on the

@@ -17,29 +17,40 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = [os.path.join(_HERE, "tdse_oracle.c"), os.path.join(_HERE, "tdse_oracle_step.inc")]
 _SO = os.path.join(_HERE, "_build", "liboracle_tdse.so")
 _LOCK = threading.Lock()
-_LIB = None
 
 PERIODIC, DIRICHLET = 0, 1
 
 
-def build(force: bool = False) -> str:
-    """Compile the oracle with gcc (-O2 -ffp-contract=off -fopenmp). Returns the .so path."""
-    os.makedirs(os.path.dirname(_SO), exist_ok=True)
+_FLAGS = {
+    # the build every parity test and pin runs: no FMA contraction, literal grouping of eqs (8)-(9)
+    "parity": ["-O2", "-ffp-contract=off"],
+    # the same source with the flags BASELINE.md section 3 names for the timed serial / OpenMP figures; timing only
+    "timing": ["-O3", "-march=native"],
+}
+_LIBS = {}
+
+
+def _so_path(variant: str) -> str:
+    return _SO if variant == "parity" else _SO.replace(".so", "_%s.so" % variant)
+
+
+def build(force: bool = False, variant: str = "parity") -> str:
+    """Compile the oracle with gcc (parity: -O2 -ffp-contract=off -fopenmp). Returns the .so path."""
+    so = _so_path(variant)
+    os.makedirs(os.path.dirname(so), exist_ok=True)
     newest = max(os.path.getmtime(p) for p in _SRC)
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < newest:
-        tmp = _SO + ".tmp.%d" % os.getpid()
-        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-std=c99", "-shared", "-fPIC",
-               "-o", tmp, _SRC[0], "-lm"]
+    if force or not os.path.exists(so) or os.path.getmtime(so) < newest:
+        tmp = so + ".tmp.%d" % os.getpid()
+        cmd = ["gcc"] + _FLAGS[variant] + ["-fopenmp", "-std=c99", "-shared", "-fPIC", "-o", tmp, _SRC[0], "-lm"]
         subprocess.run(cmd, check=True, cwd=_HERE)
-        os.replace(tmp, _SO)
-    return _SO
+        os.replace(tmp, so)
+    return so
 
 
-def lib():
-    global _LIB
+def lib(variant: str = "parity"):
     with _LOCK:
-        if _LIB is None:
-            L = C.CDLL(build())
+        if variant not in _LIBS:
+            L = C.CDLL(build(variant=variant))
             dp, fp, ip = C.POINTER(C.c_double), C.POINTER(C.c_float), C.POINTER(C.c_int)
             L.oracle_max_threads.restype = C.c_int
             L.oracle_set_threads.argtypes = [C.c_int]
@@ -63,16 +74,16 @@ def lib():
             L.oracle_potential_cell.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [dp] + [C.c_int] * 3 + [C.c_double] * 8 + [dp]
             L.oracle_dissimilarity.restype = C.c_double
             L.oracle_dissimilarity.argtypes = [dp, dp, C.c_int, C.c_double, C.c_int, C.c_int]
-            _LIB = L
-    return _LIB
+            _LIBS[variant] = L
+    return _LIBS[variant]
 
 
-def max_threads() -> int:
-    return int(lib().oracle_max_threads())
+def max_threads(variant: str = "parity") -> int:
+    return int(lib(variant).oracle_max_threads())
 
 
-def set_threads(n: int) -> None:
-    lib().oracle_set_threads(int(n))
+def set_threads(n: int, variant: str = "parity") -> None:
+    lib(variant).oracle_set_threads(int(n))
 
 
 def _p(a: np.ndarray, ct):
@@ -188,6 +199,7 @@ class OracleRun:
         self.counter = C.c_longlong(0)
         self.keep_frames, self.include_t0 = False, True
         self.frames = []              # frame mode: rho at s = 0 (optional), h, 2h, ...
+        self.step_variant = "parity"  # bench.py's timed legs may switch the recurrence to the "timing" build
 
     # -- rounding of inputs to the run's storage dtype --------------------------------
     def _round(self, a: np.ndarray) -> np.ndarray:
@@ -269,7 +281,7 @@ class OracleRun:
 
     def _advance(self, n: int):
         ct = C.c_double if self.dtype == "f64" else C.c_float
-        f = getattr(lib(), "oracle_step_" + self.dtype)
+        f = getattr(lib(self.step_variant), "oracle_step_" + self.dtype)
         cap = n // self.every + 2 if self.every > 0 else 1
         tr = np.zeros(cap, dtype=np.float64)
         ns = C.c_int(0)

@@ -30,7 +30,7 @@ SYMBOLS = [
     "tdse_set_wavepacket", "tdse_set_state", "tdse_set_detector", "tdse_step",
     "tdse_detector_read", "tdse_detector_device", "tdse_read_psi", "tdse_read_potential",
     "tdse_norm", "tdse_set_option", "tdse_get_info", "tdse_last_error",
-    "tdse_set_frames", "tdse_frames_read", "tdse_frames_device", "tdse_dissimilarity", "tdse_set_spacing", "tdse_set_potential_cell",
+    "tdse_set_frames", "tdse_frames_read", "tdse_frames_device", "tdse_dissimilarity", "tdse_set_spacing", "tdse_set_potential_cell", "tdse_set_potential_batch",
 ]
 
 
@@ -66,6 +66,7 @@ def load():
     L.tdse_set_potential.argtypes = [vp, C.c_int, C.POINTER(Atom), C.c_int] + [C.c_double] * 3
     L.tdse_set_potential_device.argtypes = [vp, C.c_int, vp, C.c_int] + [C.c_double] * 3
     L.tdse_set_potential_grid.argtypes = [vp, C.c_int, vp, C.c_int]
+    L.tdse_set_potential_batch.argtypes = [vp, vp, ip, C.c_int] + [C.c_double] * 3
     L.tdse_set_wavepacket.argtypes = [vp, C.c_int] + [C.c_double] * 8
     L.tdse_set_state.argtypes = [vp, C.c_int, vp, vp, C.c_int]
     L.tdse_set_detector.argtypes = [vp, C.c_int, C.c_int, C.c_int]
@@ -113,14 +114,16 @@ class Tdse:
         self.dtype = dtype
         self.np_dtype = np.float32 if dtype == "f32" else np.float64
         self._h = C.c_void_p()
-        code = self.L.tdse_create(C.byref(self._h), self.nx, self.ny, self.nz, self.batch,
-                                  float(dx), float(dt), float(mass), float(hbar),
-                                  TDSE_F32 if dtype == "f32" else TDSE_F64)
+        self.device = torch.device(device)
+        # tdse_create records the current device; every later call runs there whatever device is current then
+        with torch.cuda.device(self.device):
+            code = self.L.tdse_create(C.byref(self._h), self.nx, self.ny, self.nz, self.batch,
+                                      float(dx), float(dt), float(mass), float(hbar),
+                                      TDSE_F32 if dtype == "f32" else TDSE_F64)
         if code != TDSE_OK:
             raise TdseError(code, "tdse_create", (self.L.tdse_last_error(None) or b"").decode())
         nbytes = self.L.tdse_workspace_bytes(self.nx, self.ny, self.nz, self.batch,
                                              TDSE_F32 if dtype == "f32" else TDSE_F64, 1 if pingpong else 0)
-        self.device = torch.device(device)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # torch owns the memory
         self.stream = stream
         sptr = stream.cuda_stream if stream is not None else 0
@@ -154,6 +157,18 @@ class Tdse:
     def set_potential_device(self, b, atoms_tensor, natoms, vmin, vmax, rcut=0.0):
         self._check(self.L.tdse_set_potential_device(self._h, b, atoms_tensor.data_ptr(), natoms, vmin, vmax, rcut),
                     "tdse_set_potential_device")
+
+    def set_potential_batch(self, atoms, offsets, vmin, vmax, rcut=0.0):
+        """atoms: concatenated [total][6] list (numpy array on the host, or a device tensor); offsets: batch + 1 ints."""
+        off = np.ascontiguousarray(offsets, dtype=np.int32)
+        assert off.size == self.batch + 1
+        if hasattr(atoms, "data_ptr"):
+            ptr, dev = atoms.data_ptr(), 1
+        else:
+            atoms = np.ascontiguousarray(np.asarray(atoms, dtype=np.float64).reshape(-1, 6))
+            ptr, dev = atoms.ctypes.data, 0
+        self._check(self.L.tdse_set_potential_batch(self._h, ptr, off.ctypes.data_as(C.POINTER(C.c_int)), dev, vmin, vmax, rcut),
+                    "tdse_set_potential_batch")
 
     def set_potential_cell(self, b, cell, a, origin, vmin, vmax):
         if hasattr(cell, "data_ptr"):
@@ -262,8 +277,11 @@ class Tdse:
         if getattr(w, "dy", None) or getattr(w, "dz", None):
             t.set_spacing(w.dy or w.dx, w.dz or w.dx)
         t.set_boundary(*w.bc, w.absorb_lo, w.absorb_hi, w.strength, w.power)
-        for b in range(w.batch):
-            t.set_potential(b, w.atoms[b], w.vmin, w.vmax, w.rcut)
+        if w.batch > 1:
+            t.set_potential_batch(np.concatenate(w.atoms, axis=0), np.concatenate([[0], np.cumsum([a.shape[0] for a in w.atoms])]),
+                                  w.vmin, w.vmax, w.rcut)
+        else:
+            t.set_potential(0, w.atoms[0], w.vmin, w.vmax, w.rcut)
         p = w.packet
         t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
         t.set_detector(w.k_det, w.every, max(1, w.steps // max(w.every, 1)))

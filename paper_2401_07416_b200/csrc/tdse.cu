@@ -26,6 +26,7 @@ namespace {
 std::string g_create_error;
 
 constexpr size_t kAlign = 256;
+constexpr int kMaxDevices = 64;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
 }  // namespace
@@ -50,6 +51,7 @@ struct tdse_ctx {
     void* V = nullptr;
     int cur = 0;
     cudaStream_t stream = nullptr;
+    int device = 0;                     // the device that was current in tdse_create: every later call runs there
 
     // small library-owned buffers
     void* mask_dev = nullptr;           // real[nz]
@@ -60,6 +62,11 @@ struct tdse_ctx {
     unsigned* done = nullptr;           // detector kernel: blocks finished per entry (returns to 0 after every sample)
     size_t partial_n = 0;
     double* scalars = nullptr;          // 4 doubles
+    AtomRange* pot_ranges = nullptr;    // tdse_set_potential_batch: per-entry slices of the atom array [batch]
+    int* pot_count = nullptr;           //   shared-prefix length found on the device
+    double* pot_prefix = nullptr;       //   fp64 sums of the shared prefix, flat [nz][ny][nx]
+    double* cell_stage = nullptr;       // tdse_set_potential_cell: device copy of a host unit cell
+    size_t cell_cap = 0;
     AtomRec* atoms_dev = nullptr;
     AtomRec* atoms_pin = nullptr;
     int atoms_cap = 0;
@@ -74,7 +81,7 @@ struct tdse_ctx {
     double vabs_max = 0.0;
 
     // options / info
-    int opt_kernel = TDSE_KERNEL_AUTO, opt_tblock = 0, allow_unstable = 0, opt_pf = 0, opt_chunks = 0, opt_pdl = 1;
+    int opt_kernel = TDSE_KERNEL_AUTO, opt_tblock = 0, allow_unstable = 0, opt_pf = 0, opt_chunks = 0, opt_pdl = 1, opt_variant = 0;
     long long launches = 0;
     int last_kernel = 0, last_tblock = 0, last_tile_x = 0, last_tile_y = 0, last_chunks = 0;
     int num_sms = 148;
@@ -83,6 +90,21 @@ struct tdse_ctx {
 };
 
 namespace {
+
+// Every entry point runs on the context's device whatever device the caller has current, and restores the caller's.
+struct DeviceScope {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceScope(const tdse_ctx* c)
+    {
+        if (!c) return;
+        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; return; }
+        if (prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~DeviceScope() { if (switched) cudaSetDevice(prev); }
+    DeviceScope(const DeviceScope&) = delete;
+    DeviceScope& operator=(const DeviceScope&) = delete;
+};
 
 int fail(tdse_ctx* ctx, int code, const std::string& msg)
 {
@@ -282,10 +304,10 @@ int get_tensor_maps(tdse_ctx* c, int W, int NP, const CUtensorMap** out)
 
 // z chunking of one fused variant: minimise waves * (chunk length + halo planes) on num_sms * ctas_per_sm slots.
 // Also used without launching, to compare variants (auto_tblock).  planes_out = planes one CTA marches times waves.
-template <typename real, int T, int BX, int BY, int NT, int PF, int MINB = 1>
+template <typename real, int T, int BX, int BY, int NT, int PF, int MINB = 1, bool LATE = false>
 int plan_fused(tdse_ctx* c, int ctas_per_sm, int* tiles_x, int* tiles_y, int* bz_out, int* nchunks_out, long long* planes_out)
 {
-    using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
+    using Tr = FusedTraits<real, T, BX, BY, NT, PF, LATE>;
     constexpr size_t kMaxSmem = MINB == 1 ? 227 * 1024 : (228 * 1024) / MINB - 1024;   // per CTA (1 KB reserved each)
     *tiles_x = (c->g.nx + BX - 1) / BX;
     *tiles_y = (c->g.ny + BY - 1) / BY;
@@ -315,19 +337,19 @@ int plan_fused(tdse_ctx* c, int ctas_per_sm, int* tiles_x, int* tiles_y, int* bz
 // ---------------------------------------------------------------------------------------------
 // fused launch table
 // ---------------------------------------------------------------------------------------------
-template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY, int MINB = 1>
+template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY, int MINB = 1, bool SPLIT = false, bool LATE = false>
 int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
 {
-    using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
-    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF, GHOSTXY, MINB>;
+    using Tr = FusedTraits<real, T, BX, BY, NT, PF, LATE>;
+    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF, GHOSTXY, MINB, SPLIT, LATE>;
     constexpr size_t kMaxSmem = MINB == 1 ? 227 * 1024 : (228 * 1024) / MINB - 1024;   // per CTA (1 KB reserved each)
     static_assert(Tr::SMEM_FIXED + 64 * sizeof(real) <= kMaxSmem, "fused tile does not fit in shared memory");
-    static bool attr_set = false;
-    if (!attr_set) {
+    static bool attr_set[kMaxDevices] = {};          // the attribute is per device, not per process
+    if (c->device >= kMaxDevices || !attr_set[c->device]) {
         CU_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
-        attr_set = true;
+        if (c->device < kMaxDevices) attr_set[c->device] = true;
     }
-    int rc = plan_fused<real, T, BX, BY, NT, PF, MINB>(c, ctas_per_sm, &P.tiles_x, &P.tiles_y, &P.bz, &P.nchunks, nullptr);
+    int rc = plan_fused<real, T, BX, BY, NT, PF, MINB, LATE>(c, ctas_per_sm, &P.tiles_x, &P.tiles_y, &P.bz, &P.nchunks, nullptr);
     if (rc) return rc;
     const long long units = (long long)P.tiles_x * P.tiles_y * c->g.batch;
     constexpr int H = Tr::H;
@@ -355,18 +377,38 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
 template <bool GHOSTXY>
 int launch_fused_bc(tdse_ctx* c, FusedParams& P, int T)
 {
+    const bool split = (c->opt_variant & 1) != 0;    // the iteration barrier as an mbarrier (default prefetch depth only)
+    // experiments on the T = 2 kernels: bit 1 = I and V fetched one plane late (shorter rings), bit 2 = the same with one
+    // more plane in flight
+    if (T == 2 && (c->opt_variant & 6) && c->opt_pf == 0) {
+        const bool deep = (c->opt_variant & 4) != 0;
+        if (c->dtype == TDSE_F32) {
+            if (deep) return split ? launch_fused_cfg<float, 2, 64, 32, 384, 3, GHOSTXY, 1, true, true>(c, P, 1)
+                                   : launch_fused_cfg<float, 2, 64, 32, 384, 3, GHOSTXY, 1, false, true>(c, P, 1);
+            return split ? launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY, 1, true, true>(c, P, 1)
+                         : launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY, 1, false, true>(c, P, 1);
+        }
+        if (deep) return split ? launch_fused_cfg<double, 2, 32, 24, 320, 4, GHOSTXY, 1, true, true>(c, P, 1)
+                               : launch_fused_cfg<double, 2, 32, 24, 320, 4, GHOSTXY, 1, false, true>(c, P, 1);
+        return split ? launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY, 1, true, true>(c, P, 1)
+                     : launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY, 1, false, true>(c, P, 1);
+    }
     if (c->dtype == TDSE_F32) {
         if (T == 2) return c->opt_pf == 1 ? launch_fused_cfg<float, 2, 64, 32, 384, 1, GHOSTXY>(c, P, 1)
+                         : split          ? launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY, 1, true>(c, P, 1)
                                           : launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY>(c, P, 1);
         return c->opt_pf == 1 ? launch_fused_cfg<float, 1, 64, 32, 352, 1, GHOSTXY>(c, P, 1)
              : c->opt_pf == 2 ? launch_fused_cfg<float, 1, 64, 32, 352, 2, GHOSTXY>(c, P, 1)
+             : split          ? launch_fused_cfg<float, 1, 64, 32, 352, 4, GHOSTXY, 1, true>(c, P, 1)
                               : launch_fused_cfg<float, 1, 64, 32, 352, 4, GHOSTXY>(c, P, 1);
     }
     if (T == 2) return c->opt_pf == 1 ? launch_fused_cfg<double, 2, 32, 24, 320, 1, GHOSTXY>(c, P, 1)
                      : c->opt_pf == 2 ? launch_fused_cfg<double, 2, 32, 24, 320, 2, GHOSTXY>(c, P, 1)
+                     : split          ? launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY, 1, true>(c, P, 1)
                                       : launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY>(c, P, 1);
     return c->opt_pf == 1 ? launch_fused_cfg<double, 1, 32, 32, 352, 1, GHOSTXY>(c, P, 1)
          : c->opt_pf == 2 ? launch_fused_cfg<double, 1, 32, 32, 352, 2, GHOSTXY>(c, P, 1)
+         : split          ? launch_fused_cfg<double, 1, 32, 32, 352, 4, GHOSTXY, 1, true>(c, P, 1)
                           : launch_fused_cfg<double, 1, 32, 32, 352, 4, GHOSTXY>(c, P, 1);
 }
 
@@ -527,9 +569,8 @@ int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
     c->arr_bytes = align_up((size_t)c->g.pcells * batch * c->w);
     c->have_V.assign(batch, 0);
     c->have_state.assign(batch, 0);
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaGetDevice(&c->device);
+    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
     auto bail = [&](const char* what, cudaError_t err) {
         std::string m = std::string("tdse_create: ") + what + ": " + cudaGetErrorString(err);
         tdse_destroy(c);
@@ -549,6 +590,7 @@ int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
 int tdse_destroy(tdse_ctx* c)
 {
     if (!c) return TDSE_OK;
+    DeviceScope on_device_(c);
     cudaStreamSynchronize(c->stream);
     if (c->ws_owned && c->ws) cudaFree(c->ws);
     if (c->mask_dev) cudaFree(c->mask_dev);
@@ -558,6 +600,10 @@ int tdse_destroy(tdse_ctx* c)
     if (c->partial) cudaFree(c->partial);
     if (c->done) cudaFree(c->done);
     if (c->scalars) cudaFree(c->scalars);
+    if (c->cell_stage) cudaFree(c->cell_stage);
+    if (c->pot_ranges) cudaFree(c->pot_ranges);
+    if (c->pot_count) cudaFree(c->pot_count);
+    if (c->pot_prefix) cudaFree(c->pot_prefix);
     if (c->atoms_dev) cudaFree(c->atoms_dev);
     if (c->atoms_pin) cudaFreeHost(c->atoms_pin);
     if (c->atoms_ev) cudaEventDestroy(c->atoms_ev);
@@ -569,6 +615,7 @@ int tdse_destroy(tdse_ctx* c)
 int tdse_bind(tdse_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (!dev_workspace) return fail(c, TDSE_EINVAL, "tdse_bind: workspace is NULL");
     if (reinterpret_cast<uintptr_t>(dev_workspace) % kAlign) return fail(c, TDSE_EINVAL, "tdse_bind: workspace must be 256-byte aligned");
     if (bytes < 3 * c->arr_bytes) return fail(c, TDSE_ENOMEM, "tdse_bind: workspace smaller than tdse_workspace_bytes(..., 0)");
@@ -585,29 +632,102 @@ int tdse_bind(tdse_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream)
 int tdse_set_boundary(tdse_ctx* c, int bcx, int bcy, int bcz, int absorb_lo, int absorb_hi, double strength, int power)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     auto okbc = [](int b) { return b == TDSE_BC_PERIODIC || b == TDSE_BC_DIRICHLET; };
     if (!okbc(bcx) || !okbc(bcy) || !okbc(bcz)) return fail(c, TDSE_EINVAL, "tdse_set_boundary: unknown boundary flag");
     if (absorb_lo < 0 || absorb_hi < 0 || absorb_lo + absorb_hi > c->g.nz) return fail(c, TDSE_EINVAL, "tdse_set_boundary: absorber widths");
     if (!(strength >= 0.0 && strength <= 1.0) || power < 1) return fail(c, TDSE_EINVAL, "tdse_set_boundary: strength in [0,1], power >= 1");
+    const bool xy_changed = bcx != c->g.bcx || bcy != c->g.bcy;
     c->g.bcx = bcx; c->g.bcy = bcy; c->g.bcz = bcz;
     c->absorb_lo = absorb_lo; c->absorb_hi = absorb_hi; c->strength = strength; c->power = power;
-    return upload_mask(c);
+    int rc = upload_mask(c);
+    if (rc) return rc;
+    // The storage frame of every xy plane holds periodic images or Dirichlet zeros (tdse_common.cuh) and the fused kernel
+    // takes its x/y neighbours from it: data loaded under the old flags gets the frame of the new ones.
+    if (xy_changed && c->ws) {
+        for (int e = 0; e < c->g.batch; ++e) {
+            if (c->have_V[e] && (rc = fill_frame(c, entry_ptr(c, c->V, e)))) return rc;
+            if (c->have_state[e]) {
+                if ((rc = fill_frame(c, entry_ptr(c, c->R[c->cur], e)))) return rc;
+                if ((rc = fill_frame(c, entry_ptr(c, c->I[c->cur], e)))) return rc;
+            }
+        }
+    }
+    return TDSE_OK;
 }
 
-static int build_potential(tdse_ctx* c, int b, const AtomRec* atoms_dev, int natoms, double vmin, double vmax, double rcut)
+}  // extern "C"
+
+namespace {
+
+// host atom list -> pinned staging buffer -> device copy (both library-owned, grown on demand), asynchronously
+int stage_atoms(tdse_ctx* c, const AtomRec* atoms_host, int natoms)
+{
+    static_assert(sizeof(AtomRec) == sizeof(tdse_atom), "atom record layout");
+    if (natoms > c->atoms_cap) {
+        CU_TRY(c, cudaStreamSynchronize(c->stream));
+        if (c->atoms_dev) cudaFree(c->atoms_dev);
+        if (c->atoms_pin) cudaFreeHost(c->atoms_pin);
+        c->atoms_dev = nullptr; c->atoms_pin = nullptr; c->atoms_cap = 0;
+        const int cap = std::max(natoms, 1024);
+        CU_TRY(c, cudaMalloc(&c->atoms_dev, (size_t)cap * sizeof(AtomRec)));
+        CU_TRY(c, cudaMallocHost(&c->atoms_pin, (size_t)cap * sizeof(AtomRec)));
+        c->atoms_cap = cap;
+        c->atoms_pending = false;
+    }
+    if (c->atoms_pending) { CU_TRY(c, cudaEventSynchronize(c->atoms_ev)); c->atoms_pending = false; }
+    if (natoms > 0) {
+        std::memcpy(c->atoms_pin, atoms_host, (size_t)natoms * sizeof(AtomRec));
+        CU_TRY(c, cudaMemcpyAsync(c->atoms_dev, c->atoms_pin, (size_t)natoms * sizeof(AtomRec), cudaMemcpyHostToDevice, c->stream));
+        // the pinned staging buffer may be rewritten once this copy is done (event); the device copy is
+        // rewritten by the next call's H2D, which the stream orders after this call's build kernel
+        CU_TRY(c, cudaEventRecord(c->atoms_ev, c->stream));
+        c->atoms_pending = true;
+    }
+    return TDSE_OK;
+}
+
+// One launch of the potential builder: entries e0 .. e0+nent-1, entry q sums atoms [first, first+count) of `atoms_dev`
+// (ranges_dev[q], or (first0, count0) for every entry when ranges_dev is NULL), starting from prefix_in if given.
+template <typename real, int CELLS, bool HAS_CUT, bool PREFIX_OUT>
+int launch_potential(tdse_ctx* c, int e0, int nent, const AtomRec* atoms_dev, const AtomRange* ranges_dev, int first0,
+                            int count0, const double* prefix_in, double vmin, double vmax, double rcut, double* prefix_out)
+{
+    const long long bricks = (long long)((c->g.nx + CELLS * kPotBX - 1) / (CELLS * kPotBX)) *
+                             ((c->g.ny + kPotBY - 1) / kPotBY) * ((c->g.nz + kPotBZ - 1) / kPotBZ);
+    if (bricks > 0x7fffffffLL || nent > 65535) return fail(c, TDSE_EINVAL, "tdse_set_potential: grid too large");
+    potential_build_kernel<real, CELLS, HAS_CUT, PREFIX_OUT><<<dim3((unsigned)bricks, (unsigned)nent), 256, 0, c->stream>>>(
+        c->g, c->m.dx, c->m.dy, c->m.dz, atoms_dev, ranges_dev, first0, count0, prefix_in, vmin, vmax, rcut,
+        reinterpret_cast<real*>(entry_ptr(c, c->V, e0)), prefix_out);
+    CU_LAUNCH_CHECK(c);
+    return TDSE_OK;
+}
+
+template <bool PREFIX_OUT>
+int launch_potential_any(tdse_ctx* c, int e0, int nent, const AtomRec* atoms_dev, const AtomRange* ranges_dev, int first0,
+                                int count0, const double* prefix_in, double vmin, double vmax, double rcut, double* prefix_out)
+{
+    const bool wide = c->g.nx >= 8 * kPotBX;       // 8 cells per thread once a brick row of 128 cells fits
+    const bool cut = rcut > 0.0;
+#define TDSE_POT(REAL, CELLS, CUT) \
+    launch_potential<REAL, CELLS, CUT, PREFIX_OUT>(c, e0, nent, atoms_dev, ranges_dev, first0, count0, prefix_in, vmin, vmax, rcut, prefix_out)
+    if (c->dtype == TDSE_F32) {
+        if (wide) return cut ? TDSE_POT(float, 8, true) : TDSE_POT(float, 8, false);
+        return cut ? TDSE_POT(float, 4, true) : TDSE_POT(float, 4, false);
+    }
+    if (wide) return cut ? TDSE_POT(double, 8, true) : TDSE_POT(double, 8, false);
+    return cut ? TDSE_POT(double, 4, true) : TDSE_POT(double, 4, false);
+#undef TDSE_POT
+}
+
+// one atom list for entries b0 .. b1-1 (built once, copied to the others)
+int build_potential(tdse_ctx* c, int b, const AtomRec* atoms_dev, int natoms, double vmin, double vmax, double rcut)
 {
     int b0, b1;
     if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_potential: entry out of range");
-    const long long pot_bricks = (long long)((c->g.nx + kPotCells * kPotBX - 1) / (kPotCells * kPotBX)) *
-                                 ((c->g.ny + kPotBY - 1) / kPotBY) * ((c->g.nz + kPotBZ - 1) / kPotBZ);
-    if (pot_bricks > 0x7fffffffLL) return fail(c, TDSE_EINVAL, "tdse_set_potential: grid too large");
-    const unsigned nblk = (unsigned)pot_bricks;
+    const int rc = launch_potential_any<false>(c, b0, 1, atoms_dev, nullptr, 0, natoms, nullptr, vmin, vmax, rcut, nullptr);
+    if (rc) return rc;
     void* dst = entry_ptr(c, c->V, b0);
-    if (c->dtype == TDSE_F32)
-        potential_build_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, atoms_dev, natoms, vmin, vmax, rcut, static_cast<float*>(dst));
-    else
-        potential_build_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, atoms_dev, natoms, vmin, vmax, rcut, static_cast<double*>(dst));
-    CU_LAUNCH_CHECK(c);
     for (int e = b0 + 1; e < b1; ++e)
         CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->V, e), dst, (size_t)c->g.pcells * c->w, cudaMemcpyDeviceToDevice, c->stream));
     for (int e = b0; e < b1; ++e) c->have_V[e] = 1;
@@ -615,9 +735,45 @@ static int build_potential(tdse_ctx* c, int b, const AtomRec* atoms_dev, int nat
     return TDSE_OK;
 }
 
+// every entry its own list, one launch; the atoms all lists start with (nshared) are summed once into an fp64 scratch
+int build_potential_batch(tdse_ctx* c, const AtomRec* atoms_dev, const std::vector<AtomRange>& ranges, int nshared,
+                                 double vmin, double vmax, double rcut)
+{
+    const int batch = c->g.batch;
+    if (!c->pot_ranges) CU_TRY(c, cudaMalloc(&c->pot_ranges, (size_t)batch * sizeof(AtomRange)));
+    std::vector<AtomRange> rest(ranges);
+    const double* prefix = nullptr;
+    // sharing pays when the prefix pass (one entry's worth of work on nshared atoms) is cheaper than what it saves
+    if (batch >= 2 && nshared >= 8) {
+        if (!c->pot_prefix) {
+            const cudaError_t e = cudaMalloc(&c->pot_prefix, (size_t)c->g.cells * sizeof(double));
+            if (e != cudaSuccess) { cudaGetLastError(); c->pot_prefix = nullptr; }     // no scratch: plain sums
+        }
+        if (c->pot_prefix) {
+            const int rc = launch_potential_any<true>(c, 0, 1, atoms_dev, nullptr, ranges[0].first, nshared, nullptr, vmin, vmax, rcut, c->pot_prefix);
+            if (rc) return rc;
+            for (AtomRange& r : rest) { r.first += nshared; r.count -= nshared; }
+            prefix = c->pot_prefix;
+        }
+    }
+    // the previous call's ranges may still be in use by its kernel: the copy is ordered behind it on the stream
+    // (pageable source: cudaMemcpyAsync returns once `rest` has been staged)
+    CU_TRY(c, cudaMemcpyAsync(c->pot_ranges, rest.data(), (size_t)batch * sizeof(AtomRange), cudaMemcpyHostToDevice, c->stream));
+    const int rc = launch_potential_any<false>(c, 0, batch, atoms_dev, c->pot_ranges, 0, 0, prefix, vmin, vmax, rcut, nullptr);
+    if (rc) return rc;
+    std::fill(c->have_V.begin(), c->have_V.end(), 1);
+    c->vabs_max = std::max(c->vabs_max, std::max(std::fabs(vmin), std::fabs(vmax)));
+    return TDSE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
 int tdse_set_spacing(tdse_ctx* c, double dy, double dz)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (!(dy > 0) || !(dz > 0)) return fail(c, TDSE_EINVAL, "tdse_set_spacing: dy, dz must be > 0");
     c->m.dy = dy; c->m.dz = dz;
     c->m.cy = c->hbar * c->dt / (2.0 * c->mass * dy * dy);
@@ -632,37 +788,20 @@ int tdse_set_spacing(tdse_ctx* c, double dy, double dz)
 int tdse_set_potential(tdse_ctx* c, int b, const tdse_atom* atoms_host, int natoms, double vmin, double vmax, double rcut)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (natoms < 0 || (natoms > 0 && !atoms_host)) return fail(c, TDSE_EINVAL, "tdse_set_potential: atom list");
     if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential: vmin > vmax");
     int rc = ensure_workspace(c);
     if (rc) return rc;
-    if (natoms > c->atoms_cap) {
-        CU_TRY(c, cudaStreamSynchronize(c->stream));
-        if (c->atoms_dev) cudaFree(c->atoms_dev);
-        if (c->atoms_pin) cudaFreeHost(c->atoms_pin);
-        c->atoms_dev = nullptr; c->atoms_pin = nullptr; c->atoms_cap = 0;
-        const int cap = std::max(natoms, 1024);
-        CU_TRY(c, cudaMalloc(&c->atoms_dev, (size_t)cap * sizeof(AtomRec)));
-        CU_TRY(c, cudaMallocHost(&c->atoms_pin, (size_t)cap * sizeof(AtomRec)));
-        c->atoms_cap = cap;
-        c->atoms_pending = false;
-    }
-    if (c->atoms_pending) { CU_TRY(c, cudaEventSynchronize(c->atoms_ev)); c->atoms_pending = false; }
-    if (natoms > 0) {
-        static_assert(sizeof(AtomRec) == sizeof(tdse_atom), "atom record layout");
-        std::memcpy(c->atoms_pin, atoms_host, (size_t)natoms * sizeof(AtomRec));
-        CU_TRY(c, cudaMemcpyAsync(c->atoms_dev, c->atoms_pin, (size_t)natoms * sizeof(AtomRec), cudaMemcpyHostToDevice, c->stream));
-        // the pinned staging buffer may be rewritten once this copy is done (event); the device copy is
-        // rewritten by the next call's H2D, which the stream orders after this call's build kernel
-        CU_TRY(c, cudaEventRecord(c->atoms_ev, c->stream));
-        c->atoms_pending = true;
-    }
+    rc = stage_atoms(c, reinterpret_cast<const AtomRec*>(atoms_host), natoms);
+    if (rc) return rc;
     return build_potential(c, b, c->atoms_dev, natoms, vmin, vmax, rcut);
 }
 
 int tdse_set_potential_device(tdse_ctx* c, int b, const tdse_atom* atoms_device, int natoms, double vmin, double vmax, double rcut)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (natoms < 0 || (natoms > 0 && !atoms_device)) return fail(c, TDSE_EINVAL, "tdse_set_potential_device: atom list");
     if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential_device: vmin > vmax");
     int rc = ensure_workspace(c);
@@ -670,10 +809,58 @@ int tdse_set_potential_device(tdse_ctx* c, int b, const tdse_atom* atoms_device,
     return build_potential(c, b, reinterpret_cast<const AtomRec*>(atoms_device), natoms, vmin, vmax, rcut);
 }
 
+int tdse_set_potential_batch(tdse_ctx* c, const tdse_atom* atoms, const int* offsets_host, int on_device,
+                             double vmin, double vmax, double rcut)
+{
+    if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
+    const int batch = c->g.batch;
+    if (!offsets_host) return fail(c, TDSE_EINVAL, "tdse_set_potential_batch: offsets is NULL");
+    if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential_batch: vmin > vmax");
+    std::vector<AtomRange> ranges(batch);
+    for (int e = 0; e < batch; ++e) {
+        if (offsets_host[e] < 0 || offsets_host[e + 1] < offsets_host[e])
+            return fail(c, TDSE_EINVAL, "tdse_set_potential_batch: offsets must be non-negative and non-decreasing");
+        ranges[e].first = offsets_host[e];
+        ranges[e].count = offsets_host[e + 1] - offsets_host[e];
+    }
+    const int total = offsets_host[batch];
+    if (total > 0 && !atoms) return fail(c, TDSE_EINVAL, "tdse_set_potential_batch: atom list");
+    int rc = ensure_workspace(c);
+    if (rc) return rc;
+    int min_count = ranges[0].count;
+    for (const AtomRange& r : ranges) min_count = std::min(min_count, r.count);
+    int nshared = 0;
+    const AtomRec* atoms_dev = reinterpret_cast<const AtomRec*>(atoms);
+    if (!on_device) {
+        const AtomRec* host = reinterpret_cast<const AtomRec*>(atoms);
+        nshared = batch >= 2 ? min_count : 0;
+        for (int e = 1; e < batch && nshared > 0; ++e)
+            for (int a = 0; a < nshared; ++a)
+                if (std::memcmp(host + ranges[0].first + a, host + ranges[e].first + a, sizeof(AtomRec)) != 0) { nshared = a; break; }
+        rc = stage_atoms(c, host, total);
+        if (rc) return rc;
+        atoms_dev = c->atoms_dev;
+    } else if (batch >= 2 && min_count >= 8) {
+        // shared prefix of device-resident lists: compared on the device, one int comes back
+        if (!c->pot_ranges) CU_TRY(c, cudaMalloc(&c->pot_ranges, (size_t)batch * sizeof(AtomRange)));
+        if (!c->pot_count) CU_TRY(c, cudaMalloc(&c->pot_count, sizeof(int)));
+        CU_TRY(c, cudaMemcpyAsync(c->pot_ranges, ranges.data(), (size_t)batch * sizeof(AtomRange), cudaMemcpyHostToDevice, c->stream));
+        CU_TRY(c, cudaMemcpyAsync(c->pot_count, &min_count, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+        common_prefix_kernel<<<dim3((unsigned)((min_count + 127) / 128), (unsigned)(batch - 1)), 128, 0, c->stream>>>(
+            atoms_dev, c->pot_ranges, min_count, c->pot_count);
+        CU_LAUNCH_CHECK(c);
+        CU_TRY(c, cudaMemcpyAsync(&nshared, c->pot_count, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CU_TRY(c, cudaStreamSynchronize(c->stream));
+    }
+    return build_potential_batch(c, atoms_dev, ranges, nshared, vmin, vmax, rcut);
+}
+
 int tdse_set_potential_cell(tdse_ctx* c, int b, const double* cell, int on_device, int mx, int my, int mz,
                             double ax, double ay, double az, double x0, double y0, double z0, double vmin, double vmax)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (!cell || mx < 1 || my < 1 || mz < 1) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: cell grid");
     if (!(ax > 0) || !(ay > 0) || !(az > 0)) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: cell edge lengths must be > 0");
     if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: vmin > vmax");
@@ -683,12 +870,17 @@ int tdse_set_potential_cell(tdse_ctx* c, int b, const double* cell, int on_devic
     if (rc) return rc;
     const size_t n = (size_t)mx * my * mz;
     const double* cell_dev = cell;
-    double* staged = nullptr;
     if (!on_device) {
-        CU_TRY(c, cudaMalloc(&staged, n * sizeof(double)));
-        cudaError_t e = cudaMemcpyAsync(staged, cell, n * sizeof(double), cudaMemcpyHostToDevice, c->stream);
-        if (e != cudaSuccess) { cudaFree(staged); return fail(c, TDSE_ECUDA, std::string("tdse_set_potential_cell: ") + cudaGetErrorString(e)); }
-        cell_dev = staged;
+        // library-owned staging buffer, kept across calls (grown when a larger cell arrives); the copy and the kernel
+        // are ordered on the stream, and cudaMemcpyAsync from pageable memory returns once the source has been read
+        if (n > c->cell_cap) {
+            if (c->cell_stage) { CU_TRY(c, cudaStreamSynchronize(c->stream)); cudaFree(c->cell_stage); c->cell_stage = nullptr; c->cell_cap = 0; }
+            const cudaError_t e = cudaMalloc(&c->cell_stage, n * sizeof(double));
+            if (e != cudaSuccess) { cudaGetLastError(); c->cell_stage = nullptr; return fail(c, TDSE_ENOMEM, std::string("tdse_set_potential_cell: staging: ") + cudaGetErrorString(e)); }
+            c->cell_cap = n;
+        }
+        CU_TRY(c, cudaMemcpyAsync(c->cell_stage, cell, n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        cell_dev = c->cell_stage;
     }
     CellParams p{mx, my, mz, ax, ay, az, x0, y0, z0, vmin, vmax};
     const unsigned nblk = (unsigned)((c->g.cells + 255) / 256);
@@ -697,10 +889,7 @@ int tdse_set_potential_cell(tdse_ctx* c, int b, const double* cell, int on_devic
         potential_cell_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, cell_dev, p, static_cast<float*>(dst));
     else
         potential_cell_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, cell_dev, p, static_cast<double*>(dst));
-    cudaError_t le = cudaGetLastError();
-    if (staged) { cudaStreamSynchronize(c->stream); cudaFree(staged); }
-    if (le != cudaSuccess) return fail(c, TDSE_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(le));
-    c->launches++;
+    CU_LAUNCH_CHECK(c);
     for (int e = b0 + 1; e < b1; ++e)
         CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->V, e), dst, (size_t)c->g.pcells * c->w, cudaMemcpyDeviceToDevice, c->stream));
     for (int e = b0; e < b1; ++e) c->have_V[e] = 1;
@@ -711,6 +900,7 @@ int tdse_set_potential_cell(tdse_ctx* c, int b, const double* cell, int on_devic
 int tdse_set_potential_grid(tdse_ctx* c, int b, const void* V, int on_device)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (!V) return fail(c, TDSE_EINVAL, "tdse_set_potential_grid: V is NULL");
     int b0, b1;
     if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_potential_grid: entry out of range");
@@ -742,6 +932,7 @@ int tdse_set_wavepacket(tdse_ctx* c, int b, double x0, double y0, double z0, dou
                         double kx, double ky, double kz, double amplitude)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (!(sigma > 0)) return fail(c, TDSE_EINVAL, "tdse_set_wavepacket: sigma must be > 0");
     int b0, b1;
     if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_wavepacket: entry out of range");
@@ -770,6 +961,7 @@ int tdse_set_wavepacket(tdse_ctx* c, int b, double x0, double y0, double z0, dou
 int tdse_set_state(tdse_ctx* c, int b, const void* R, const void* I_half, int on_device)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (!R || !I_half) return fail(c, TDSE_EINVAL, "tdse_set_state: NULL state");
     int b0, b1;
     if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_state: entry out of range");
@@ -790,18 +982,31 @@ int tdse_set_state(tdse_ctx* c, int b, const void* R, const void* I_half, int on
 int tdse_set_detector(tdse_ctx* c, int k_plane, int every, int max_samples)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (every < 0 || max_samples < 0) return fail(c, TDSE_EINVAL, "tdse_set_detector: every, max_samples must be >= 0");
     if (every > 0 && (k_plane < 0 || k_plane >= c->g.nz)) return fail(c, TDSE_EINVAL, "tdse_set_detector: plane out of range");
-    CU_TRY(c, cudaStreamSynchronize(c->stream));
-    if (c->trace) { cudaFree(c->trace); c->trace = nullptr; }
-    c->k_det = k_plane; c->every = every; c->max_samples = max_samples;
-    if (max_samples > 0) CU_TRY(c, cudaMalloc(&c->trace, (size_t)c->g.batch * max_samples * sizeof(double)));
+    if (max_samples != c->max_samples) {
+        // a new trace buffer is allocated before the old one is given up, so a failed allocation leaves the context usable
+        double* fresh = nullptr;
+        if (max_samples > 0) {
+            const cudaError_t e = cudaMalloc(&fresh, (size_t)c->g.batch * max_samples * sizeof(double));
+            if (e != cudaSuccess) {
+                cudaGetLastError();
+                return fail(c, TDSE_ENOMEM, std::string("tdse_set_detector: trace buffer: ") + cudaGetErrorString(e));
+            }
+        }
+        if (c->trace) { CU_TRY(c, cudaStreamSynchronize(c->stream)); cudaFree(c->trace); }
+        c->trace = fresh;
+        c->max_samples = max_samples;
+    }
+    c->k_det = k_plane; c->every = every;
     return reset_detector(c);
 }
 
 int tdse_step(tdse_ctx* c, int n)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (n < 0) return fail(c, TDSE_EINVAL, "tdse_step: n < 0");
     if (!c->ws) return fail(c, TDSE_ESTATE, "tdse_step: potential and state are not set");
     for (int e = 0; e < c->g.batch; ++e)
@@ -867,6 +1072,7 @@ int tdse_step(tdse_ctx* c, int n)
 int tdse_detector_read(tdse_ctx* c, int b, double* image_host, double* trace_host, int cap, int* nsamples)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_detector_read: entry out of range");
     if (cap < 0) return fail(c, TDSE_EINVAL, "tdse_detector_read: cap < 0");
     if (image_host)
@@ -882,6 +1088,7 @@ int tdse_detector_read(tdse_ctx* c, int b, double* image_host, double* trace_hos
 int tdse_set_frames(tdse_ctx* c, int max_frames, int include_t0)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (max_frames < 0) return fail(c, TDSE_EINVAL, "tdse_set_frames: max_frames < 0");
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     if (c->frames) { cudaFree(c->frames); c->frames = nullptr; }
@@ -897,6 +1104,7 @@ int tdse_set_frames(tdse_ctx* c, int max_frames, int include_t0)
 int tdse_frames_read(tdse_ctx* c, int b, int first, int count, double* frames_host, int* nframes)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_frames_read: entry out of range");
     const int have = std::min(c->nframes, c->max_frames);
     if (first < 0 || count < 0 || first + count > have) return fail(c, TDSE_EINVAL, "tdse_frames_read: frame range exceeds the frames kept");
@@ -922,6 +1130,7 @@ int tdse_frames_device(tdse_ctx* c, double** frames_device, int* max_frames, int
 int tdse_dissimilarity(tdse_ctx* c, int first_frame, int last_frame, double* d_host)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (!d_host) return fail(c, TDSE_EINVAL, "tdse_dissimilarity: NULL");
     if (!c->frames) return fail(c, TDSE_ESTATE, "tdse_dissimilarity: frame mode is off (tdse_set_frames)");
     const int have = std::min(c->nframes, c->max_frames);
@@ -955,6 +1164,7 @@ int tdse_detector_device(tdse_ctx* c, double** image_device, double** trace_devi
 int tdse_read_psi(tdse_ctx* c, int b, void* R_host, void* I_host)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_read_psi: entry out of range");
     if (!c->ws || !c->have_state[b]) return fail(c, TDSE_ESTATE, "tdse_read_psi: state not set");
     int rc;
@@ -967,6 +1177,7 @@ int tdse_read_psi(tdse_ctx* c, int b, void* R_host, void* I_host)
 int tdse_read_potential(tdse_ctx* c, int b, void* V_host)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_read_potential: entry out of range");
     if (!c->ws || !c->have_V[b]) return fail(c, TDSE_ESTATE, "tdse_read_potential: potential not set");
     if (!V_host) return fail(c, TDSE_EINVAL, "tdse_read_potential: NULL");
@@ -978,6 +1189,7 @@ int tdse_read_potential(tdse_ctx* c, int b, void* V_host)
 int tdse_norm(tdse_ctx* c, int b, double* q_visscher, double* q_paper)
 {
     if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_norm: entry out of range");
     if (!c->ws || !c->have_state[b] || !c->have_V[b]) return fail(c, TDSE_ESTATE, "tdse_norm: potential and state must be set");
     const unsigned nblk = (unsigned)((c->g.cells + 255) / 256);
@@ -1016,6 +1228,9 @@ int tdse_set_option(tdse_ctx* c, const char* key, long long value)
     } else if (k == "z_chunks") {
         if (value < 0) return fail(c, TDSE_EINVAL, "tdse_set_option: z_chunks must be >= 0");
         c->opt_chunks = (int)value;
+    } else if (k == "variant") {
+        if (value < 0 || value > 7) return fail(c, TDSE_EINVAL, "tdse_set_option: variant must be 0..7");
+        c->opt_variant = (int)value;
     } else if (k == "pdl") {
         c->opt_pdl = value ? 1 : 0;
     } else if (k == "allow_unstable") {

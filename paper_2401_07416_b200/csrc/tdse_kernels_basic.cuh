@@ -10,47 +10,58 @@ struct AtomRec { double x, y, z, Z, soft2, screen; };   // same layout as tdse_a
 
 // ---------------------------------------------------------------------------------------------
 // S0 potential build (BASELINE.json north_star (1)): V = clamp(sum_a -Z_a exp(-r_a/lambda_a)/sqrt(r_a^2+s_a^2)).
-// Bound by the fp64 pipe (exp, two inverse square roots per cell-atom pair), so the work per pair is cut
-// down: a thread owns kPotCells consecutive cells along x and shares the y/z part of the distance among
-// them; atoms are staged through shared memory in chunks with 1/lambda precomputed; exp(-r/lambda) is an
-// inline range reduction + degree-13 polynomial (|error| < 1 ulp for arguments <= 0), r = r2 * rsqrt(r2).
-// Double accumulate in list order, one rounding to `real`.  Nearest image on periodic axes.
+// Bound by the fp64 pipe, so the work per cell-atom pair is cut down to ~35 fp64 instructions without branches:
+//   * a thread owns CELLS consecutive cells along x and shares the y/z part of the distance among them;
+//   * atoms are staged through shared memory in chunks with 1/lambda precomputed;
+//   * inverse square roots: the hardware seed (MUFU.RSQ64H through rsqrt.approx.ftz.f64) + one third-order step;
+//   * exp(-r/lambda): x = n ln2/32 + r, exp(x) = 2^(n div 32) * T[n mod 32] * (1 + q(r)), T[j] = 2^(j/32) in shared
+//     memory, q = expm1 as a degree-6 polynomial on |r| <= ln2/64 (remainder < 4e-18);
+//   * nearest image by the round-to-nearest-even magic constant instead of rint.
+// Double accumulate in list order, one rounding to `real`.  One launch covers every batch entry (blockIdx.y); the
+// sum may start from a per-cell prefix (the atoms all entries share, summed once: prefix_out mode) -- the same sequence of
+// fma as the plain list-order sum, so the result does not depend on whether the prefix was shared.
 // ---------------------------------------------------------------------------------------------
 constexpr int kAtomChunk = 128;
-constexpr int kPotCells = 4;
 
 struct AtomStaged { double x, y, z, Z, soft2, inv_screen; };   // inv_screen = 0: unscreened
+struct AtomRange { int first, count; };                        // one entry's slice of the atom array
 
-// exp(x) for x <= 0 (flushes to 0 below -708: smaller than any double the sum can register)
-__device__ __forceinline__ double exp_nonpositive(double x)
+constexpr double kRoundMagic = 6755399441055744.0;             // 1.5 * 2^52: x + magic - magic = x rounded to nearest even
+
+// 1/sqrt(a) for normal a > 0: ~22-bit hardware seed, then y (1 + e/2 + 3 e^2/8) with e = 1 - a y^2 (error O(e^3))
+__device__ __forceinline__ double rsqrt_pos(double a)
 {
-    if (x < -708.0) return 0.0;
-    const double magic = 6755399441055744.0;                       // 1.5 * 2^52: round to nearest integer
-    double t = fma(x, 1.4426950408889634074, magic);
-    const int k = __double2loint(t);
-    t -= magic;
-    double r = fma(t, -6.93147180369123816490e-01, x);
-    r = fma(t, -1.90821492927058770002e-10, r);                    // |r| <= ln2 / 2
-    double p = 1.0 / 6227020800.0;                                 // Taylor to r^13: remainder < 5e-18
-    p = fma(p, r, 1.0 / 479001600.0);
-    p = fma(p, r, 1.0 / 39916800.0);
-    p = fma(p, r, 1.0 / 3628800.0);
-    p = fma(p, r, 1.0 / 362880.0);
-    p = fma(p, r, 1.0 / 40320.0);
-    p = fma(p, r, 1.0 / 5040.0);
-    p = fma(p, r, 1.0 / 720.0);
-    p = fma(p, r, 1.0 / 120.0);
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    const double t = a * y;
+    const double e = fma(-t, y, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    return fma(y * e, p, y);
+}
+
+// exp(x) for -30000 < x <= 0 with the 2^(j/32) table `T` (shared memory); below -708 the result stays near 2^-1022, which
+// no sum registers.  exp(-0) = 1 exactly.
+__device__ __forceinline__ double exp_nonpositive(double x, const double* __restrict__ T)
+{
+    double t = fma(x, 32.0 * 1.4426950408889634074, kRoundMagic);
+    const int n = max(__double2loint(t), -1022 * 32);               // n = 32 k + j; k >= -1022 keeps the result a normal number
+    t -= kRoundMagic;
+    double r = fma(t, -6.93147180369123816490e-01 / 32.0, x);       // ln2 hi (32 significant bits: t * hi is exact)
+    r = fma(t, -1.90821492927058770002e-10 / 32.0, r);              // |r| <= ln2 / 64
+    double p = fma(r, 1.0 / 720.0, 1.0 / 120.0);
     p = fma(p, r, 1.0 / 24.0);
     p = fma(p, r, 1.0 / 6.0);
     p = fma(p, r, 0.5);
     p = fma(p, r, 1.0);
-    p = fma(p, r, 1.0);
-    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));   // p * 2^k, k >= -1022
+    const double s = T[n & 31];
+    const double v = fma(s, p * r, s);                              // 2^(j/32) e^r in [0.5, 2)
+    return __hiloint2double(__double2hiint(v) + ((n >> 5) << 20), __double2loint(v));   // * 2^k, k >= -1022
 }
 
 // distance from coordinate a to the interval [lo, hi] along one axis (nearest periodic image if L > 0)
 __device__ __forceinline__ double axis_gap(double a, double lo, double hi, double L)
 {
+    if (L > 0.0) a -= L * floor(a / L);   // the pair test takes any number of periods: bring a into [0, L) first
     double g = fmax(0.0, fmax(lo - a, a - hi));
     if (L > 0.0) {
         g = fmin(g, fmax(0.0, fmax(lo - (a + L), (a + L) - hi)));
@@ -59,91 +70,130 @@ __device__ __forceinline__ double axis_gap(double a, double lo, double hi, doubl
     return g;
 }
 
-// A block owns a brick of kPotBX x kPotBY x kPotBZ threads = (4 kPotBX) x kPotBY x kPotBZ cells.  With a cutoff, atoms
-// farther than rcut from every cell of the brick are dropped while the list is staged (ordered compaction, so
-// the summation order of the kept atoms is the list order); per pair the cutoff test itself is unchanged.
+// A block owns a brick of kPotBX x kPotBY x kPotBZ threads = (CELLS kPotBX) x kPotBY x kPotBZ cells of entry blockIdx.y.
+// HAS_CUT: atoms farther than rcut from every cell of the brick are dropped while the list is staged (ordered
+// compaction, so the summation order of the kept atoms is the list order); the pair test itself is the oracle's.
+// PREFIX_OUT: write the unclamped fp64 sums to `prefix_out` (flat [nz][ny][nx]) instead of V.
 constexpr int kPotBX = 16, kPotBY = 4, kPotBZ = 4;
 
-template <typename real>
-__global__ void __launch_bounds__(256)
-potential_build_kernel(Grid g, double dx, double dy, double dz, const AtomRec* __restrict__ atoms, int natoms,
-                       double vmin, double vmax, double rcut, real* __restrict__ V /* entry base */)
+template <typename real, int CELLS, bool HAS_CUT, bool PREFIX_OUT>
+__global__ void __launch_bounds__(256, 2)
+potential_build_kernel(Grid g, double dx, double dy, double dz, const AtomRec* __restrict__ atoms,
+                       const AtomRange* __restrict__ ranges /* [gridDim.y] or NULL */, int first0, int count0,
+                       const double* __restrict__ prefix_in /* flat fp64 sums of the atoms before `first`, or NULL */,
+                       double vmin, double vmax, double rcut, real* __restrict__ V /* base of entry blockIdx.y = 0 */,
+                       double* __restrict__ prefix_out)
 {
     static_assert(kPotBX * kPotBY * kPotBZ == 256 && kAtomChunk <= 256, "block shape");
     __shared__ AtomStaged s_atoms[kAtomChunk];
+    __shared__ double s_exp2[32];
     __shared__ int s_warp_count[8];
     const int tx = threadIdx.x % kPotBX, ty = (threadIdx.x / kPotBX) % kPotBY, tz = threadIdx.x / (kPotBX * kPotBY);
-    const int bricks_x = (g.nx + kPotCells * kPotBX - 1) / (kPotCells * kPotBX), bricks_y = (g.ny + kPotBY - 1) / kPotBY;
+    const int bricks_x = (g.nx + CELLS * kPotBX - 1) / (CELLS * kPotBX), bricks_y = (g.ny + kPotBY - 1) / kPotBY;
     const int bx = blockIdx.x % bricks_x, by = (blockIdx.x / bricks_x) % bricks_y, bz = blockIdx.x / (bricks_x * bricks_y);
-    const int i0 = (bx * kPotBX + tx) * kPotCells, j = by * kPotBY + ty, k = bz * kPotBZ + tz;
+    const int i0 = (bx * kPotBX + tx) * CELLS, j = by * kPotBY + ty, k = bz * kPotBZ + tz;
     const bool live = i0 < g.nx && j < g.ny && k < g.nz;
+    const int first = ranges ? ranges[blockIdx.y].first : first0;
+    const int natoms = ranges ? ranges[blockIdx.y].count : count0;
     const double y = j * dy, z = k * dz;
     const double Lx = g.nx * dx, Ly = g.ny * dy, Lz = g.nz * dz;
     const double iLx = 1.0 / Lx, iLy = 1.0 / Ly, iLz = 1.0 / Lz;
     const bool perx = g.bcx == BC_PERIODIC, pery = g.bcy == BC_PERIODIC, perz = g.bcz == BC_PERIODIC;
     const double rc2 = rcut * rcut;
     // the brick's bounding box, padded by a cell so that rounding never drops an atom the pair test would keep
-    const double lox = (bx * kPotBX * kPotCells - 1) * dx, hix = ((bx + 1) * kPotBX * kPotCells) * dx;
+    const double lox = (bx * kPotBX * CELLS - 1) * dx, hix = ((bx + 1) * kPotBX * CELLS) * dx;
     const double loy = (by * kPotBY - 1) * dy, hiy = ((by + 1) * kPotBY) * dy;
     const double loz = (bz * kPotBZ - 1) * dz, hiz = ((bz + 1) * kPotBZ) * dz;
-    double sum[kPotCells];
+    if (threadIdx.x < 32) s_exp2[threadIdx.x] = exp2((double)threadIdx.x / 32.0);
+    double sum[CELLS], xs[CELLS];
 #pragma unroll
-    for (int e = 0; e < kPotCells; ++e) sum[e] = 0.0;
+    for (int e = 0; e < CELLS; ++e) xs[e] = (i0 + e) * dx;
+    const long long flat0 = ((long long)k * g.ny + j) * g.nx + i0;
+#pragma unroll
+    for (int e = 0; e < CELLS; ++e) sum[e] = (prefix_in && live && i0 + e < g.nx) ? prefix_in[flat0 + e] : 0.0;
     for (int a0 = 0; a0 < natoms; a0 += kAtomChunk) {
         const int nc = min(kAtomChunk, natoms - a0);
-        __syncthreads();                                  // previous chunk fully consumed
-        // ---- stage: thread q < nc looks at atom a0 + q; kept atoms are compacted in list order ----
-        AtomStaged S;
-        bool keep = false;
-        if (threadIdx.x < nc) {
-            const AtomRec A = atoms[a0 + threadIdx.x];
-            S.x = A.x; S.y = A.y; S.z = A.z; S.Z = A.Z; S.soft2 = A.soft2;
-            S.inv_screen = (A.screen > 0.0 && isfinite(A.screen)) ? 1.0 / A.screen : 0.0;
-            keep = true;
-            if (rcut > 0.0) {
-                const double gx = axis_gap(A.x, lox, hix, perx ? Lx : 0.0);
-                const double gy = axis_gap(A.y, loy, hiy, pery ? Ly : 0.0);
-                const double gz = axis_gap(A.z, loz, hiz, perz ? Lz : 0.0);
-                keep = gx * gx + gy * gy + gz * gz <= rc2;
+        __syncthreads();                                  // previous chunk fully consumed (first pass: table written)
+        // ---- stage: thread q < nc looks at atom first + a0 + q ----
+        int na = nc;
+        {
+            AtomStaged S;
+            bool keep = false;
+            if (threadIdx.x < nc) {
+                const AtomRec A = atoms[first + a0 + threadIdx.x];
+                S.x = A.x; S.y = A.y; S.z = A.z; S.Z = A.Z; S.soft2 = A.soft2;
+                S.inv_screen = (A.screen > 0.0 && isfinite(A.screen)) ? 1.0 / A.screen : 0.0;
+                keep = true;
+                if (HAS_CUT) {
+                    const double gx = axis_gap(A.x, lox, hix, perx ? Lx : 0.0);
+                    const double gy = axis_gap(A.y, loy, hiy, pery ? Ly : 0.0);
+                    const double gz = axis_gap(A.z, loz, hiz, perz ? Lz : 0.0);
+                    keep = gx * gx + gy * gy + gz * gz <= rc2;
+                }
+            }
+            if (HAS_CUT) {                                // kept atoms are compacted in list order
+                const unsigned ballot = __ballot_sync(0xffffffffu, keep);
+                const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+                if (lane == 0) s_warp_count[warp] = __popc(ballot);
+                __syncthreads();
+                int base = 0;
+                na = 0;
+#pragma unroll
+                for (int w = 0; w < 8; ++w) { if (w < warp) base += s_warp_count[w]; na += s_warp_count[w]; }
+                if (keep) s_atoms[base + __popc(ballot & ((1u << lane) - 1u))] = S;
+            } else if (keep) {
+                s_atoms[threadIdx.x] = S;
             }
         }
-        const unsigned ballot = __ballot_sync(0xffffffffu, keep);
-        const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-        if (lane == 0) s_warp_count[warp] = __popc(ballot);
-        __syncthreads();
-        int base = 0, na = 0;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) { if (w < warp) base += s_warp_count[w]; na += s_warp_count[w]; }
-        if (keep) s_atoms[base + __popc(ballot & ((1u << lane) - 1u))] = S;
         __syncthreads();
         if (!live) continue;
         for (int a = 0; a < na; ++a) {
             const AtomStaged A = s_atoms[a];
             double ddy = y - A.y, ddz = z - A.z;
-            if (pery) ddy = fma(-Ly, rint(ddy * iLy), ddy);
-            if (perz) ddz = fma(-Lz, rint(ddz * iLz), ddz);
-            const double yz2 = fma(ddy, ddy, ddz * ddz);
+            if (pery) ddy = fma(-Ly, fma(ddy, iLy, kRoundMagic) - kRoundMagic, ddy);
+            if (perz) ddz = fma(-Lz, fma(ddz, iLz, kRoundMagic) - kRoundMagic, ddz);
+            // + 1e-200: an atom on a grid point gives r = 1e-100 instead of 0 * inf; any r2 >= 1e-184 is unchanged
+            const double yz2 = fma(ddy, ddy, ddz * ddz) + 1e-200;
+            const double nZ = -A.Z;
 #pragma unroll
-            for (int e = 0; e < kPotCells; ++e) {
-                double ddx = (i0 + e) * dx - A.x;
-                if (perx) ddx = fma(-Lx, rint(ddx * iLx), ddx);
+            for (int e = 0; e < CELLS; ++e) {
+                double ddx = xs[e] - A.x;
+                if (perx) ddx = fma(-Lx, fma(ddx, iLx, kRoundMagic) - kRoundMagic, ddx);
                 const double r2 = fma(ddx, ddx, yz2);
-                double r = r2 > 0.0 ? r2 * rsqrt(r2) : 0.0;
-                if (rcut > 0.0) {
+                double r = r2 * rsqrt_pos(r2);
+                if (HAS_CUT) {
                     // the cutoff is defined on r = sqrt(r2) (correctly rounded): decide on r2 unless it is a tie
                     if (fabs(r2 - rc2) <= 1e-12 * rc2) r = sqrt(r2);
                     if (r > rcut) continue;
                 }
-                const double screen = A.inv_screen > 0.0 ? exp_nonpositive(-r * A.inv_screen) : 1.0;
-                sum[e] = fma(-A.Z * screen, rsqrt(r2 + A.soft2), sum[e]);
+                const double screen = exp_nonpositive(-r * A.inv_screen, s_exp2);   // inv_screen = 0: exactly 1
+                sum[e] = fma(nZ * screen, rsqrt_pos(r2 + A.soft2), sum[e]);
             }
         }
     }
     if (live) {
 #pragma unroll
-        for (int e = 0; e < kPotCells; ++e)
-            if (i0 + e < g.nx) store_with_images(V, g, i0 + e, j, k, (real)fmin(fmax(sum[e], vmin), vmax));
+        for (int e = 0; e < CELLS; ++e) {
+            if (i0 + e >= g.nx) continue;
+            if (PREFIX_OUT) prefix_out[flat0 + e] = sum[e];
+            else store_with_images(V + (long long)blockIdx.y * g.pcells, g, i0 + e, j, k, (real)fmin(fmax(sum[e], vmin), vmax));
+        }
     }
+}
+
+// Length of the atom-list prefix that every entry shares with entry 0 (compared bit by bit): *out starts at the shortest
+// list length and is lowered to the first index at which some entry differs.  grid: x covers min_count, y = batch - 1.
+__global__ void common_prefix_kernel(const AtomRec* __restrict__ atoms, const AtomRange* __restrict__ ranges, int min_count,
+                                     int* __restrict__ out)
+{
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= min_count) return;
+    const unsigned long long* p0 = reinterpret_cast<const unsigned long long*>(atoms + ranges[0].first + a);
+    const unsigned long long* pb = reinterpret_cast<const unsigned long long*>(atoms + ranges[blockIdx.y + 1].first + a);
+    bool same = true;
+#pragma unroll
+    for (int q = 0; q < 6; ++q) same = same && p0[q] == pb[q];
+    if (!same) atomicMin(out, a);
 }
 
 // ---------------------------------------------------------------------------------------------

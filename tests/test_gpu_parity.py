@@ -269,6 +269,18 @@ def test_fused_and_twopass_agree_and_conserve_the_visscher_norm():
 # ------------------------------------------------------------------------------------------
 # the BASELINE configurations (reduced grid / full steps where the oracle finishes in seconds)
 # ------------------------------------------------------------------------------------------
+# per-cell guard beside the rel-L2 bound (a single wrong seam cell of a 512^3 grid moves the rel-L2 by < 1e-4):
+# max |error| over all cells, relative to max |psi| (for the image: to max D)
+CELL_TOL = {"f64": 1e-10, "f32": 1e-3}
+
+
+def max_abs_rel(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    scale = float(np.max(np.abs(b)))
+    return float(np.max(np.abs(a - b))) / scale if scale > 0 else float(np.max(np.abs(a)))
+
+
 def _run_config(w, steps, entries=None):
     from paper_2401_07416_b200 import Tdse
     t = Tdse.from_workload(w)
@@ -281,6 +293,8 @@ def _run_config(w, steps, entries=None):
         errs = (rel_l2(R, o.R), rel_l2(I, o.I), rel_l2(D, o.D), rel_l2(tr, o.trace))
         worst = max(worst, *errs)
         assert len(tr) == len(o.trace) == steps // w.every
+        cell = max(max_abs_rel(R, o.R), max_abs_rel(I, o.I), max_abs_rel(D, o.D))
+        assert cell < CELL_TOL[w.dtype], "entry %d: per-cell error %.3e" % (b, cell)
     info = (t.get_info("kernel"), t.get_info("tblock"))
     t.close()
     return worst, info
@@ -354,42 +368,34 @@ def test_config4_reduced_grid_full_step_count(dtype):
     assert info == (FUSED, 2) and worst < TOL[dtype]
 
 
-@pytest.mark.skipif(not os.environ.get("TDSE_FULL_PARITY"), reason="minutes of oracle time; run with TDSE_FULL_PARITY=1 "
-                    "(results of the round-1 run: profiles/r01_full_size_parity.md)")
+@pytest.mark.skipif(bool(os.environ.get("TDSE_SKIP_FULL_PARITY")), reason="TDSE_SKIP_FULL_PARITY set (minutes of oracle time)")
 @pytest.mark.parametrize("idx,dtype", [(2, "f32"), (4, "f64"), (4, "f32")])
 def test_full_size_full_step_count(idx, dtype):
     """cfg 2 (256 x 256 x 512 f32, 8000 steps) and cfg 4 (384^3 f64 and 512^3 f32, 2000 steps, entry 0) at
-    BASELINE.json's full size and step count, every cell compared; prints the errors for the evidence file.
-
-    cfg 4 at 512^3 in f32 is the one case where the detector image cannot meet 1e-4, for a reason that has nothing to do
-    with the kernel: the recipe puts the packet 5.4 sigma from the detector plane and 2000 steps move it by 6.4 bohr,
-    so the plane only ever sees the Gaussian tail (density 1e-13 of the peak), and after ~1500 steps float rounding
-    noise radiated by the packet arrives there.  The oracle's own float instantiation shows the same: the bound
-    asserted for that image is 3 x (oracle-f32 vs oracle-f64) on the same z geometry, measured here on a 64 x 64 x 512 box."""
+    BASELINE.json's full size and step count, every cell compared (rel-L2 and per-cell); prints the errors for the
+    evidence file (profiles/r02_full_size_parity.md).  The oracle needs minutes of host time per case (OpenMP);
+    TDSE_SKIP_FULL_PARITY=1 leaves these three out of a quick local run."""
+    import time
     from paper_2401_07416_b200 import Tdse
     w = make_config(idx, dtype=dtype, batch=1) if idx == 4 else make_config(idx)
+    t0 = time.time()
     t = Tdse.from_workload(w)
     t.step(w.steps)
     R, I = t.read_psi(0)
     D, tr = t.detector_read(0)
     info = (t.get_info("kernel"), t.get_info("tblock"))
     t.close()
+    t1 = time.time()
     o = oracle_for(w, 0, w.steps)
+    t2 = time.time()
     e_psi = max(rel_l2(R, o.R), rel_l2(I, o.I))
     e_det = max(rel_l2(D, o.D), rel_l2(tr, o.trace))
-    det_tol = TOL[dtype]
-    note = ""
-    if (idx, dtype) == (4, "f32"):
-        ws = make_config(4, dtype="f32", batch=1, n=(64, 64, w.nz))
-        o64 = OracleRun.from_workload(ws, dtype="f64", round_to="f32").step(ws.steps)
-        o32 = OracleRun.from_workload(ws, dtype="f32").step(ws.steps)
-        floor = max(rel_l2(o32.D, o64.D), rel_l2(o32.trace, o64.trace))
-        det_tol = max(det_tol, 3.0 * floor)
-        note = "; float noise floor of the detector on this z geometry (oracle-f32 vs oracle-f64, 64x64x%d): %.3e" % (w.nz, floor)
-    print("full-size parity cfg%d %s %dx%dx%d, %d steps: rel-L2 psi %.3e, detector image/trace %.3e (kernel %s)%s"
-          % (idx, dtype, w.nx, w.ny, w.nz, w.steps, e_psi, e_det, info, note))
+    e_cell = max(max_abs_rel(R, o.R), max_abs_rel(I, o.I), max_abs_rel(D, o.D))
+    print("full-size parity cfg%d %s %dx%dx%d, %d steps: rel-L2 psi %.3e, detector image/trace %.3e, per-cell %.3e "
+          "(kernel %s; GPU %.0f s, oracle %.0f s on %d threads)"
+          % (idx, dtype, w.nx, w.ny, w.nz, w.steps, e_psi, e_det, e_cell, info, t1 - t0, t2 - t1, oracle.max_threads()))
     assert info == (FUSED, 2)
-    assert e_psi < TOL[dtype] and e_det < det_tol
+    assert e_psi < TOL[dtype] and e_det < TOL[dtype] and e_cell < CELL_TOL[dtype]
 
 
 # ------------------------------------------------------------------------------------------
@@ -731,3 +737,172 @@ def test_user_stream_and_device_resident_inputs():
         o = oracle_for(w, b, 40)
         assert rel_l2(R, o.R) < 1e-4 and rel_l2(D, o.D) < 1e-4 and rel_l2(tr, o.trace) < 1e-4
     t.close()
+
+
+# ------------------------------------------------------------------------------------------
+# call order, devices, buffers (host-side logic of the library)
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel,tblock", VARIANTS)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("first,then", [((PERIODIC, PERIODIC, DIRICHLET), (DIRICHLET, DIRICHLET, DIRICHLET)),
+                                        ((DIRICHLET, DIRICHLET, DIRICHLET), (PERIODIC, PERIODIC, PERIODIC)),
+                                        ((PERIODIC, DIRICHLET, PERIODIC), (DIRICHLET, PERIODIC, DIRICHLET))])
+def test_boundary_flags_changed_after_the_data_was_loaded(kernel, tblock, dtype, first, then):
+    """tdse_set_boundary after tdse_set_state / tdse_set_potential_grid: the fused kernel takes its x/y neighbours from
+    the storage frames, which were filled under the old flags and must follow the new ones (include/tdse.h)."""
+    nx, ny, nz, dx, dt, steps = 40, 24, 18, 0.25, 0.004, 9
+    t = make_ctx(nx, ny, nz, 1, dx, dt, dtype)
+    t.set_boundary(*first, 3, 3, 0.07, 2)
+    t.set_option("kernel", kernel)
+    t.set_option("tblock", tblock)
+    V = random_potential(300, (nz, ny, nx), -30.0, 5.0)
+    R0, I0 = random_state(301, (nz, ny, nx))
+    t.set_potential_grid(0, V.astype(t.np_dtype))
+    t.set_state(0, R0.astype(t.np_dtype), I0.astype(t.np_dtype))
+    t.set_boundary(*then, 3, 3, 0.07, 2)
+    t.set_detector(2, 3, 4)
+    t.step(steps)
+    o = OracleRun(nx, ny, nz, dx, dt, bc=then, absorb_lo=3, absorb_hi=3, strength=0.07,
+                  round_to="f32" if dtype == "f32" else None)
+    o.set_potential_grid(V).set_state(R0, I0).set_detector(2, 3).step(steps)
+    R, I = t.read_psi(0)
+    D, tr = t.detector_read(0)
+    tol = TOL[dtype]
+    assert t.get_info("kernel") == kernel
+    assert rel_l2(R, o.R) < tol and rel_l2(I, o.I) < tol and rel_l2(D, o.D) < tol and rel_l2(tr, o.trace) < tol
+    t.close()
+
+
+def test_atoms_many_periods_outside_the_box_with_a_cutoff():
+    """The pair test takes the nearest image over any number of periods; the brick culling of the builder must keep
+    the same atoms (an atom three box lengths outside a periodic axis is as close as its image inside)."""
+    from paper_2401_07416_b200 import Tdse
+    w = make_config(4, n=(48, 40, 56), batch=1, dtype="f64")
+    lx, ly = w.nx * w.dx, w.ny * w.dx
+    atoms = w.atoms[0].copy()
+    atoms[::3, 0] += 3.0 * lx
+    atoms[1::3, 1] -= 2.0 * ly
+    w2 = w.with_(atoms=[atoms], rcut=3.0)
+    t = Tdse.from_workload(w2)
+    V = t.read_potential(0)
+    t.close()
+    o = OracleRun.from_workload(w2, entry=0, dtype="f64")
+    o_in = OracleRun.from_workload(w.with_(rcut=3.0), entry=0, dtype="f64")
+    assert np.max(np.abs(V - o.V64)) <= 1e-13 * max(1.0, np.max(np.abs(o.V64)))
+    assert np.max(np.abs(o.V64 - o_in.V64)) <= 1e-9 * np.max(np.abs(o_in.V64))     # the shifted list is the same crystal
+
+
+def test_set_detector_keeps_the_trace_buffer_and_survives_a_failed_allocation():
+    from paper_2401_07416_b200 import Tdse, TdseError, TDSE_ENOMEM
+    w = make_config(0, n=(24, 24, 24), steps=0, batch=64)
+    t = Tdse.from_workload(w)
+    t.set_detector(5, 2, 6)
+    _, tr0, ms0 = t.detector_device()
+    t.step(4)
+    t.set_detector(7, 2, 6)                        # same max_samples: same buffer, counters reset
+    _, tr1, ms1 = t.detector_device()
+    assert tr0 == tr1 and ms0 == ms1 == 6 and t.get_info("nsamples") == 0
+    with pytest.raises(TdseError) as e:
+        t.set_detector(7, 2, 2 ** 31 - 1)          # 64 entries x 16 GiB of doubles: beyond any device
+    assert e.value.code == TDSE_ENOMEM
+    _, tr2, ms2 = t.detector_device()
+    assert tr2 == tr1 and ms2 == 6                 # the previous set-up is still in force
+    t.step(4)
+    D, tr = t.detector_read(0)
+    o = OracleRun.from_workload(w).step(4).set_detector(7, 2).step(4)      # set_detector resets image, trace and counter only
+    assert len(tr) == 2 and rel_l2(D, o.D) < 1e-12 and rel_l2(tr, o.trace) < 1e-12
+    t.close()
+
+
+def test_contexts_on_two_devices_in_one_process():
+    """cudaFuncSetAttribute is per device and every call must run on its context's device whatever is current."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    from paper_2401_07416_b200 import Tdse
+    w = make_config(1, n=(32, 32, 40), steps=0)
+    ctxs = [Tdse.from_workload(w, device="cuda:%d" % d) for d in (0, 1)]
+    torch.cuda.set_device(0)
+    for t in ctxs:
+        t.step(20)
+    o = OracleRun.from_workload(w).step(20)
+    for t in ctxs:
+        assert t.get_info("kernel") == FUSED
+        R, I = t.read_psi(0)
+        assert rel_l2(R, o.R) < 1e-11 and rel_l2(I, o.I) < 1e-11
+        t.close()
+    assert torch.cuda.current_device() == 0
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("idx,shape,batch", [(3, (36, 40, 44), 5), (3, (128, 24, 20), 3), (4, (48, 40, 56), 3), (2, (40, 36, 48), 2)])
+def test_batched_potential_build_is_bit_identical_to_one_entry_at_a_time(idx, shape, batch, dtype):
+    """tdse_set_potential_batch (one launch, shared substrate prefix summed once, host or device lists) against
+    tdse_set_potential entry by entry: the same list-order fp64 sums, so every bit agrees; entry 0 and the last entry
+    against the oracle as well.  Shapes cover both cells-per-thread variants (nx >= 128) and the cutoff variant (cfg 4)."""
+    import torch
+    from paper_2401_07416_b200 import Tdse
+    w = make_config(idx, n=shape, batch=batch, dtype=dtype)
+    if idx == 4:
+        w = w.with_(atoms=[w.atoms[0]] + [np.concatenate([w.atoms[0][:9], a[9:]]) for a in w.atoms[1:]])   # shared prefix of 9 atoms together with the cutoff
+    cat = np.ascontiguousarray(np.concatenate(w.atoms, axis=0))
+    off = np.concatenate([[0], np.cumsum([a.shape[0] for a in w.atoms])]).astype(np.int32)
+    ref = make_ctx(w.nx, w.ny, w.nz, batch, w.dx, w.dt, dtype)
+    ref.set_boundary(*w.bc, w.absorb_lo, w.absorb_hi, w.strength, w.power)
+    for b in range(batch):
+        ref.set_potential(b, w.atoms[b], w.vmin, w.vmax, w.rcut)
+    Vref = [ref.read_potential(b) for b in range(batch)]
+    ref.close()
+    for on_device in (False, True):
+        t = make_ctx(w.nx, w.ny, w.nz, batch, w.dx, w.dt, dtype)
+        t.set_boundary(*w.bc, w.absorb_lo, w.absorb_hi, w.strength, w.power)
+        lists = torch.from_numpy(cat).cuda() if on_device else cat
+        t.set_potential_batch(lists, off, w.vmin, w.vmax, w.rcut)
+        for b in range(batch):
+            assert np.array_equal(t.read_potential(b), Vref[b]), (on_device, b)
+        # the framed storage too: the step kernel reads V through its periodic images
+        p = w.packet
+        t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], 0.0)
+        t.step(6)
+        R, _ = t.read_psi(batch - 1)
+        o = oracle_for(w, batch - 1, 6)
+        assert rel_l2(R, o.R) < TOL[dtype]
+        t.close()
+    for b in (0, batch - 1):
+        o = OracleRun.from_workload(w, entry=b, dtype="f64", round_to="f32" if dtype == "f32" else None)
+        if dtype == "f64":
+            assert np.max(np.abs(Vref[b] - o.V64)) <= 1e-13 * max(1.0, np.max(np.abs(o.V64)))
+        else:
+            ulp = np.spacing(np.abs(o.V).astype(np.float32)).astype(np.float64)
+            assert np.all(np.abs(Vref[b].astype(np.float64) - o.V) <= ulp)
+
+
+@pytest.mark.parametrize("tblock", [1, 2])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape,bc,batch", [((72, 40, 37), BCS[0], 2), ((136, 70, 21), BCS[3], 1), ((64, 64, 16), BCS[1], 3),
+                                            ((128, 128, 40), BCS[2], 2), ((40, 24, 5), BCS[4], 1)])
+def test_iteration_barrier_variants_are_bit_identical(tblock, dtype, shape, bc, batch):
+    """tdse_set_option("variant"): the fused kernel with the per-plane block barrier (0) and with the split
+    arrive / wait mbarrier (1) do the same arithmetic in the same order -- every bit of psi and of the detector output
+    must agree, over several z chunks and launches; variant 0 is the one compared with the oracle everywhere else."""
+    nx, ny, nz = shape
+    dx, dt, steps = 0.25, 0.004, 14
+    out = []
+    for variant in (0, 1):
+        t = make_ctx(nx, ny, nz, batch, dx, dt, dtype)
+        t.set_boundary(*bc, min(4, nz // 3), min(4, nz // 3), 0.07, 2)
+        t.set_option("kernel", FUSED)
+        t.set_option("tblock", tblock)
+        t.set_option("variant", variant)
+        t.set_detector(min(3, nz - 1), 4, 8)
+        for b in range(batch):
+            V = random_potential(500 + b, (nz, ny, nx), -30.0, 5.0)
+            R0, I0 = random_state(600 + b, (nz, ny, nx))
+            t.set_potential_grid(b, V.astype(t.np_dtype))
+            t.set_state(b, R0.astype(t.np_dtype), I0.astype(t.np_dtype))
+        t.step(steps)
+        out.append([t.read_psi(b) + t.detector_read(b) for b in range(batch)])
+        t.close()
+    for b in range(batch):
+        for x0, x1 in zip(out[0][b], out[1][b]):
+            assert np.array_equal(x0, x1)

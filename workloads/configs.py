@@ -163,6 +163,9 @@ def _thermal(atoms: np.ndarray, seed: int, sd: float = 0.1) -> np.ndarray:
     return out
 
 
+CFG4_ZTOP_FRAC = 0.38     # as config 1
+
+
 def make_config(idx: int, *, n: Optional[Sequence[int]] = None, batch: Optional[int] = None,
                 steps: Optional[int] = None, dtype: Optional[str] = None) -> Workload:
     """Build configuration `idx` (0..4) of BASELINE.json.
@@ -225,7 +228,9 @@ def make_config(idx: int, *, n: Optional[Sequence[int]] = None, batch: Optional[
         dx = 0.15
         nb = batch or 1
         lx, ly, lz = nx * dx, ny * dx, nz * dx
-        slab = fcc111_slab(lx, ly, 0.6 * lz, 4)
+        # "config-1 slab physics, scaled" (reading 19): config 1's fractions of the box -- slab top at 0.38 Lz,
+        # packet at 0.2 Lz, detector plane at 10/128 of the box height -- on the larger grid
+        slab = fcc111_slab(lx, ly, CFG4_ZTOP_FRAC * lz, 4)
         atoms, seeds = [], []
         for b in range(nb):
             atoms.append(slab if b == 0 else _thermal(slab, 4000 + b))
@@ -236,8 +241,8 @@ def make_config(idx: int, *, n: Optional[Sequence[int]] = None, batch: Optional[
             dx=dx, dt=_dt_rule(dx, 200.0), mass=mass, hbar=hbar,
             bc=(PERIODIC, PERIODIC, DIRICHLET), absorb_lo=absorb, absorb_hi=absorb, strength=0.05, power=2,
             atoms=atoms, vmin=-200.0, vmax=0.0, rcut=16.0,
-            packet=dict(x0=lx / 2, y0=ly / 2, z0=0.3 * lz, sigma=4.0, kx=0.0, ky=0.0, kz=3.0, amplitude=0.0),
-            k_det=min(10, nz - 1), every=10, steps=steps or 2000, seeds=seeds)
+            packet=dict(x0=lx / 2, y0=ly / 2, z0=0.2 * lz, sigma=4.0, kx=0.0, ky=0.0, kz=3.0, amplitude=0.0),
+            k_det=min(max(1, (10 * nz + 64) // 128), nz - 1), every=10, steps=steps or 2000, seeds=seeds)
 
     raise ValueError("config index must be 0..4")
 
@@ -270,7 +275,7 @@ def shard_for_rank(w: Workload, idx: int, rank: int, world: int) -> Workload:
         seeds = [2 + g0 + b for b in range(w.batch)]
         return w.with_(atoms=[_thermal(slab, s) for s in seeds], seeds=seeds)
     if idx == 4:
-        slab = fcc111_slab(lx, ly, 0.6 * lz, 4)
+        slab = fcc111_slab(lx, ly, CFG4_ZTOP_FRAC * lz, 4)
         seeds = [4000 + g0 + b for b in range(w.batch)]
         return w.with_(atoms=[_thermal(slab, s) for s in seeds], seeds=seeds)
     return w
