@@ -226,6 +226,8 @@ int tdse_norm(tdse_ctx* ctx, int b, double* q_visscher, double* q_paper);
  * "z_chunks" (z chunks per tile column in the fused launch, 0 = chosen by the launcher),
  * "pdl" (0/1, default 1: fused launches carry the programmatic-stream-serialization attribute, so the next
  * launch becomes resident while the previous one drains; results are bit-identical either way),
+ * "variant" (0 = the launcher decides, 1 / 2 = force on / off the fused kernel whose per-plane block barrier is a split
+ * arrive / wait mbarrier; same arithmetic in the same order, so results are bit-identical),
  * "allow_unstable" (0/1).  Errors: TDSE_EINVAL for unknown keys or values. */
 int tdse_set_option(tdse_ctx* ctx, const char* key, long long value);
 

@@ -304,10 +304,10 @@ int get_tensor_maps(tdse_ctx* c, int W, int NP, const CUtensorMap** out)
 
 // z chunking of one fused variant: minimise waves * (chunk length + halo planes) on num_sms * ctas_per_sm slots.
 // Also used without launching, to compare variants (auto_tblock).  planes_out = planes one CTA marches times waves.
-template <typename real, int T, int BX, int BY, int NT, int PF, int MINB = 1, bool LATE = false>
+template <typename real, int T, int BX, int BY, int NT, int PF, int MINB = 1>
 int plan_fused(tdse_ctx* c, int ctas_per_sm, int* tiles_x, int* tiles_y, int* bz_out, int* nchunks_out, long long* planes_out)
 {
-    using Tr = FusedTraits<real, T, BX, BY, NT, PF, LATE>;
+    using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
     constexpr size_t kMaxSmem = MINB == 1 ? 227 * 1024 : (228 * 1024) / MINB - 1024;   // per CTA (1 KB reserved each)
     *tiles_x = (c->g.nx + BX - 1) / BX;
     *tiles_y = (c->g.ny + BY - 1) / BY;
@@ -337,11 +337,11 @@ int plan_fused(tdse_ctx* c, int ctas_per_sm, int* tiles_x, int* tiles_y, int* bz
 // ---------------------------------------------------------------------------------------------
 // fused launch table
 // ---------------------------------------------------------------------------------------------
-template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY, int MINB = 1, bool SPLIT = false, bool LATE = false>
+template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY, int MINB = 1, bool SPLIT = false>
 int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
 {
-    using Tr = FusedTraits<real, T, BX, BY, NT, PF, LATE>;
-    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF, GHOSTXY, MINB, SPLIT, LATE>;
+    using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
+    auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF, GHOSTXY, MINB, SPLIT>;
     constexpr size_t kMaxSmem = MINB == 1 ? 227 * 1024 : (228 * 1024) / MINB - 1024;   // per CTA (1 KB reserved each)
     static_assert(Tr::SMEM_FIXED + 64 * sizeof(real) <= kMaxSmem, "fused tile does not fit in shared memory");
     static bool attr_set[kMaxDevices] = {};          // the attribute is per device, not per process
@@ -349,7 +349,7 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
         CU_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
         if (c->device < kMaxDevices) attr_set[c->device] = true;
     }
-    int rc = plan_fused<real, T, BX, BY, NT, PF, MINB, LATE>(c, ctas_per_sm, &P.tiles_x, &P.tiles_y, &P.bz, &P.nchunks, nullptr);
+    int rc = plan_fused<real, T, BX, BY, NT, PF, MINB>(c, ctas_per_sm, &P.tiles_x, &P.tiles_y, &P.bz, &P.nchunks, nullptr);
     if (rc) return rc;
     const long long units = (long long)P.tiles_x * P.tiles_y * c->g.batch;
     constexpr int H = Tr::H;
@@ -374,42 +374,41 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
     return TDSE_OK;
 }
 
+// The iteration barrier as a split arrive / wait mbarrier (SPLIT, tdse_kernels_fused.cuh) pays where a launch is a single wave
+// of short z chunks, i.e. where skew between warps is not hidden by other CTAs' work queued behind: measured +5 % on one
+// 128^3 f64 grid, +2 % on 64^3 f64, -1..2 % on every multi-wave grid and on the f32 kernels (profiles/README.md, round 2).
+// tdse_set_option("variant", 1 | 2) forces it on | off.
+template <typename real, int T, int BX, int BY, int NT, int PF>
+bool want_split(tdse_ctx* c)
+{
+    if (c->opt_variant == 1) return true;
+    if (c->opt_variant == 2) return false;
+    if (sizeof(real) != 8) return false;
+    int tx, ty, bz, nch;
+    if (plan_fused<real, T, BX, BY, NT, PF>(c, 1, &tx, &ty, &bz, &nch, nullptr)) return false;
+    return (long long)tx * ty * nch * c->g.batch <= c->num_sms;
+}
+
 template <bool GHOSTXY>
 int launch_fused_bc(tdse_ctx* c, FusedParams& P, int T)
 {
-    const bool split = (c->opt_variant & 1) != 0;    // the iteration barrier as an mbarrier (default prefetch depth only)
-    // experiments on the T = 2 kernels: bit 1 = I and V fetched one plane late (shorter rings), bit 2 = the same with one
-    // more plane in flight
-    if (T == 2 && (c->opt_variant & 6) && c->opt_pf == 0) {
-        const bool deep = (c->opt_variant & 4) != 0;
-        if (c->dtype == TDSE_F32) {
-            if (deep) return split ? launch_fused_cfg<float, 2, 64, 32, 384, 3, GHOSTXY, 1, true, true>(c, P, 1)
-                                   : launch_fused_cfg<float, 2, 64, 32, 384, 3, GHOSTXY, 1, false, true>(c, P, 1);
-            return split ? launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY, 1, true, true>(c, P, 1)
-                         : launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY, 1, false, true>(c, P, 1);
-        }
-        if (deep) return split ? launch_fused_cfg<double, 2, 32, 24, 320, 4, GHOSTXY, 1, true, true>(c, P, 1)
-                               : launch_fused_cfg<double, 2, 32, 24, 320, 4, GHOSTXY, 1, false, true>(c, P, 1);
-        return split ? launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY, 1, true, true>(c, P, 1)
-                     : launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY, 1, false, true>(c, P, 1);
-    }
     if (c->dtype == TDSE_F32) {
         if (T == 2) return c->opt_pf == 1 ? launch_fused_cfg<float, 2, 64, 32, 384, 1, GHOSTXY>(c, P, 1)
-                         : split          ? launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY, 1, true>(c, P, 1)
-                                          : launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY>(c, P, 1);
+                         : want_split<float, 2, 64, 32, 384, 2>(c) ? launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY, 1, true>(c, P, 1)
+                                                                   : launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY>(c, P, 1);
         return c->opt_pf == 1 ? launch_fused_cfg<float, 1, 64, 32, 352, 1, GHOSTXY>(c, P, 1)
              : c->opt_pf == 2 ? launch_fused_cfg<float, 1, 64, 32, 352, 2, GHOSTXY>(c, P, 1)
-             : split          ? launch_fused_cfg<float, 1, 64, 32, 352, 4, GHOSTXY, 1, true>(c, P, 1)
-                              : launch_fused_cfg<float, 1, 64, 32, 352, 4, GHOSTXY>(c, P, 1);
+             : want_split<float, 1, 64, 32, 352, 4>(c) ? launch_fused_cfg<float, 1, 64, 32, 352, 4, GHOSTXY, 1, true>(c, P, 1)
+                                                       : launch_fused_cfg<float, 1, 64, 32, 352, 4, GHOSTXY>(c, P, 1);
     }
     if (T == 2) return c->opt_pf == 1 ? launch_fused_cfg<double, 2, 32, 24, 320, 1, GHOSTXY>(c, P, 1)
                      : c->opt_pf == 2 ? launch_fused_cfg<double, 2, 32, 24, 320, 2, GHOSTXY>(c, P, 1)
-                     : split          ? launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY, 1, true>(c, P, 1)
-                                      : launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY>(c, P, 1);
+                     : want_split<double, 2, 32, 24, 320, 3>(c) ? launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY, 1, true>(c, P, 1)
+                                                                : launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY>(c, P, 1);
     return c->opt_pf == 1 ? launch_fused_cfg<double, 1, 32, 32, 352, 1, GHOSTXY>(c, P, 1)
          : c->opt_pf == 2 ? launch_fused_cfg<double, 1, 32, 32, 352, 2, GHOSTXY>(c, P, 1)
-         : split          ? launch_fused_cfg<double, 1, 32, 32, 352, 4, GHOSTXY, 1, true>(c, P, 1)
-                          : launch_fused_cfg<double, 1, 32, 32, 352, 4, GHOSTXY>(c, P, 1);
+         : want_split<double, 1, 32, 32, 352, 4>(c) ? launch_fused_cfg<double, 1, 32, 32, 352, 4, GHOSTXY, 1, true>(c, P, 1)
+                                                    : launch_fused_cfg<double, 1, 32, 32, 352, 4, GHOSTXY>(c, P, 1);
 }
 
 int launch_fused(tdse_ctx* c, FusedParams& P, int T)
@@ -1229,7 +1228,7 @@ int tdse_set_option(tdse_ctx* c, const char* key, long long value)
         if (value < 0) return fail(c, TDSE_EINVAL, "tdse_set_option: z_chunks must be >= 0");
         c->opt_chunks = (int)value;
     } else if (k == "variant") {
-        if (value < 0 || value > 7) return fail(c, TDSE_EINVAL, "tdse_set_option: variant must be 0..7");
+        if (value < 0 || value > 2) return fail(c, TDSE_EINVAL, "tdse_set_option: variant must be 0 (auto), 1 or 2");
         c->opt_variant = (int)value;
     } else if (k == "pdl") {
         c->opt_pdl = value ? 1 : 0;

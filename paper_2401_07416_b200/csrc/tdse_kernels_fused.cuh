@@ -96,12 +96,9 @@ __device__ __forceinline__ void st_global_pred(void* p, const Pack<double>& v, i
                  ::"l"(p), "d"(v.e[0]), "d"(v.e[1]), "r"(pred) : "memory");
 }
 
-// LATE: planes of I and V are fetched one iteration after the R plane of the same z (stage 1 needs R of plane p but I and V
-// of plane p-1 only), so their rings are one slot shorter.
-template <typename real, int T_, int BX_, int BY_, int NT_, int PF_, bool LATE_ = false>
+template <typename real, int T_, int BX_, int BY_, int NT_, int PF_>
 struct FusedTraits {
     static constexpr int T = T_, BX = BX_, BY = BY_, NT = NT_, PF = PF_;
-    static constexpr bool LATE = LATE_;
     static constexpr int VW = 16 / sizeof(real);
     static constexpr int NS = 2 * T;                           // stages per launch
     static constexpr int H = 2 * T;                            // halo (cells) in y, planes in z
@@ -118,9 +115,8 @@ struct FusedTraits {
     static constexpr unsigned BOX_BYTES = (unsigned)(PS * sizeof(real));        // bytes one box (W x NP x 2) delivers
     static_assert((PS * sizeof(real)) % 128 == 0, "ring slots must stay 128-byte aligned for TMA");
     static constexpr int RD = PF + 2;                          // ring depth (planes p+PF .. p+1 in flight, p, p-1)
-    static constexpr int RDIV = LATE ? RD - 1 : RD;            // ring depth of I and V
     static constexpr int XD = 2;                               // exchange planes per stage (written at t, read at t+1)
-    static constexpr int NPLANES = RD + 2 * RDIV + (NS - 1) * XD;
+    static constexpr int NPLANES = 3 * RD + (NS - 1) * XD;
     static constexpr size_t SMEM_FIXED = ((size_t)NPLANES * PS + 2 * GUARD) * sizeof(real) + 128 /*alignment slack*/ + 64 /*mbarriers*/;
     // + (bz + 2H + 2) mask values, added by the launcher
     static_assert(RD <= 7, "mbarrier block holds 8 barriers: RD ring slots + the iteration barrier of the SPLIT variant");
@@ -143,24 +139,25 @@ struct Queue {                       // one z-plane worth of per-thread pipeline
 // SPLIT: the block barrier per plane becomes an mbarrier that a warp arrives at once its shared-memory traffic of
 // the iteration is done and waits for only when it needs the others' exchange planes in the next iteration; the work in
 // between (global stores, the wait for the next plane, the ring loads and all of stage 1, which needs no exchange
-// plane) absorbs the skew between warps instead of idling at a barrier.
-template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY, int MINB = 1, bool SPLIT = false, bool LATE = false>
+// plane) absorbs the skew between warps instead of idling at a barrier.  Same arithmetic, same order: bit-identical.
+// Worth 2-5 % where a launch is one wave of short chunks (64^3, one 128^3 f64 grid), nothing on the multi-wave grids.
+template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY, int MINB = 1, bool SPLIT = false>
 __global__ void __launch_bounds__(NT, MINB)
 fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
                   const __grid_constant__ CUtensorMap tmI, const __grid_constant__ CUtensorMap tmV)
 {
-    using Tr = FusedTraits<real, T, BX, BY, NT, PF, LATE>;
+    using Tr = FusedTraits<real, T, BX, BY, NT, PF>;
     using V4 = Pack<real>;
     using Q = Queue<real, Tr::NS>;
     constexpr int VW = Tr::VW, NS = Tr::NS, H = Tr::H, HX = Tr::HX, WQ = Tr::WQ, W = Tr::W;
-    constexpr int G2 = Tr::G2, PS = Tr::PS, HP = Tr::HP, RD = Tr::RD, RDIV = Tr::RDIV, XD = Tr::XD;
+    constexpr int G2 = Tr::G2, PS = Tr::PS, HP = Tr::HP, RD = Tr::RD, XD = Tr::XD;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     unsigned char* const smem_al = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);   // TMA wants 128-byte aligned boxes
     real* const ringR = reinterpret_cast<real*>(smem_al) + Tr::GUARD;
     real* const ringI = ringR + RD * PS;
-    real* const ringV = ringI + RDIV * PS;
-    real* const exch = ringV + RDIV * PS;                    // stage s output of iteration t at exch[((s-1)*XD + t%2) * PS]
+    real* const ringV = ringI + RD * PS;
+    real* const exch = ringV + RD * PS;                    // stage s output of iteration t at exch[((s-1)*XD + t%2) * PS]
     unsigned long long* const full = reinterpret_cast<unsigned long long*>(exch + (NS - 1) * XD * PS + Tr::GUARD);   // full[slot]: plane landed
     unsigned long long* const iter_done = full + 7;        // SPLIT: one arrival per warp and iteration
     real* const smask = reinterpret_cast<real*>(full + 8); // smask[q] = mask of plane Z0-H-1+q
@@ -227,19 +224,17 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
     // ---- TMA producer (thread 0): plane pz_next -> ring slot, two half-plane boxes per array ---------
     int pz_next = Z0 - H;                            // next plane to stage (wrapped when z is periodic)
     if (P.bcz == BC_PERIODIC) pz_next = wrap_index(pz_next, P.nz);
-    int pz_iv = Z0 - H - (LATE ? 1 : 0);             // next plane of I and V (LATE: one behind R)
-    if (P.bcz == BC_PERIODIC) pz_iv = wrap_index(pz_iv, P.nz);
     const int box_x = X0 - HX + PADX, box_yp = (Y0 - H + PADY) / 2;   // box origin: x, row pair (Y0-H+PADY is even)
-    auto issue_plane = [&](int ring_off, int iv_off, int slot_idx) {
+    auto issue_plane = [&](int ring_off, int slot_idx) {
         // a Dirichlet ghost plane has an out-of-range z coordinate: the TMA unit fills the box with zeros
         unsigned long long* bar = full + slot_idx;
         mbar_expect_tx(bar, 3u * Tr::BOX_BYTES);
-        tma_load_5d(ringR + ring_off, &tmR, bar, box_x, box_yp, 0, pz_next, b);
-        tma_load_5d(ringI + iv_off, &tmI, bar, box_x, box_yp, 0, pz_iv, b);
-        tma_load_5d(ringV + iv_off, &tmV, bar, box_x, box_yp, 0, pz_iv, b);
-        ++pz_next; ++pz_iv;
+        real* dst = ringR + ring_off;
+        tma_load_5d(dst, &tmR, bar, box_x, box_yp, 0, pz_next, b);
+        tma_load_5d(dst + RD * PS, &tmI, bar, box_x, box_yp, 0, pz_next, b);
+        tma_load_5d(dst + 2 * RD * PS, &tmV, bar, box_x, box_yp, 0, pz_next, b);
+        ++pz_next;
         if (P.bcz == BC_PERIODIC && pz_next == P.nz) pz_next = 0;
-        if (P.bcz == BC_PERIODIC && pz_iv == P.nz) pz_iv = 0;
     };
 
     const int niter = bzc + 2 * H;                   // planes Z0-H .. Z0+bzc+H-1 enter the pipeline
@@ -285,15 +280,13 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
     asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
     if (tid == 0) {
 #pragma unroll
-        for (int t = 0; t < PF; ++t) if (t < niter) issue_plane(t * PS, t * PS, t);
+        for (int t = 0; t < PF; ++t) if (t < niter) issue_plane(t * PS, t);
     }
     __syncthreads();                                 // barriers initialised before anyone waits on them
     // ring slot offsets (elements) of plane p (cur), p-1 (prev) and of the slot plane p+PF goes to (fill);
     // exchange-plane offsets written this iteration (xw) and read from the previous one (xr)
     auto ring_next = [](int o) { return (o + PS == RD * PS) ? 0 : o + PS; };
-    auto ring_next_iv = [](int o) { return (o + PS == RDIV * PS) ? 0 : o + PS; };
     int ro_cur = 0, ro_prev = (RD - 1) * PS, ro_fill = (PF % RD) * PS;
-    int io_cur = 0, io_fill = (PF % RDIV) * PS;      // LATE: slot of the I, V planes that landed with plane p (they are planes p-1)
     int sl_cur = 0, sl_fill = PF % RD;               // the same as slot indices (barrier array)
     unsigned par = 0;                                // phase parity of full[sl_cur]
     unsigned dpar = 0;                               // SPLIT: phase parity of iter_done
@@ -328,7 +321,7 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
         if (!SPLIT) {
             __syncthreads();                         // everyone is done with iteration t-1 (ring slot p-2, exchange planes)
             // refill the slot of plane p-2: its last readers passed the barrier above (reads ordered before the async write)
-            if (tid == 0 && t + PF < niter) issue_plane(ro_fill, LATE ? io_fill : ro_fill, sl_fill);
+            if (tid == 0 && t + PF < niter) issue_plane(ro_fill, sl_fill);
         }
 
         const int p = Z0 - H + t;
@@ -342,8 +335,8 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
         for (int j = 0; j < 2; ++j) {
             if (NS > 3) dg_oldest[j] = nw.dg[j];     // created three iterations ago: plane p-4
             nw.f[0][j] = *reinterpret_cast<const V4*>(ringR + ro_cur + soff + j * HP);
-            iold[j] = *reinterpret_cast<const V4*>(ringI + (LATE ? io_cur : ro_prev) + soff + j * HP);
-            const V4 vraw = *reinterpret_cast<const V4*>(ringV + (LATE ? io_cur : ro_prev) + soff + j * HP);
+            iold[j] = *reinterpret_cast<const V4*>(ringI + ro_prev + soff + j * HP);
+            const V4 vraw = *reinterpret_cast<const V4*>(ringV + ro_prev + soff + j * HP);
 #pragma unroll
             for (int e = 0; e < VW; ++e) nw.dg[j].e[e] = fma(cv, vraw.e[e], c2);
         }
@@ -355,7 +348,7 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
                 // in iteration t-1 and overwrites the ones they read then: wait until every warp has arrived for t-1.
                 if (t > 0) { mbar_wait(iter_done, dpar); dpar ^= 1u; }
                 // the same arrivals say that the ring slot of plane p-2 has been read for the last time: refill it
-                if (tid == 0 && t + PF < niter) issue_plane(ro_fill, LATE ? io_fill : ro_fill, sl_fill);
+                if (tid == 0 && t + PF < niter) issue_plane(ro_fill, sl_fill);
 #pragma unroll
                 for (int j = 0; j < 2; ++j) *reinterpret_cast<V4*>(exch + xw + soff + j * HP) = nw.f[1][j];
             }
@@ -418,7 +411,6 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
         }
         out_pb += plane_bytes;
         ro_prev = ro_cur; ro_cur = ring_next(ro_cur); ro_fill = ring_next(ro_fill);
-        if (LATE) { io_cur = ring_next_iv(io_cur); io_fill = ring_next_iv(io_fill); }
         if (++sl_cur == RD) { sl_cur = 0; par ^= 1u; }
         if (++sl_fill == RD) sl_fill = 0;
         xr = xw; xw = PS - xw;
