@@ -197,6 +197,21 @@ int tdse_frames_read(tdse_ctx* ctx, int b, int first, int count, double* frames_
 /* Device pointer of the frame buffer (library-owned; valid until tdse_set_frames / tdse_destroy). */
 int tdse_frames_device(tdse_ctx* ctx, double** frames_device, int* max_frames, int* nframes);
 
+/* Streamed frame mode (a 5000-step run keeps 250 frames per configuration, 879 configurations): the same
+ * frames as tdse_set_frames, but the device holds only a ring of `ring_slots` (>= 2) sample slots [slot][batch][ny][nx]; as
+ * soon as a sample's slot is written it is copied (one asynchronous strided copy per slot, on a second stream owned by
+ * the library) into `frames_host`, a HOST buffer of batch * capacity * ny * nx doubles laid out [batch][capacity][ny][nx]
+ * (page-locked memory lets the copies overlap the stepping; pageable memory works but serialises).  The stepping stream
+ * waits only when it comes back to a slot whose copy has not left yet.  Frames beyond `capacity` are dropped.  The buffer
+ * belongs to the caller and must stay valid until tdse_frames_sync has returned after the last step (or the mode is
+ * switched off with capacity = 0).  Excludes tdse_set_frames / tdse_dissimilarity (which need the frames on the device).
+ * Resets the detector.  Errors: TDSE_EINVAL, TDSE_ENOMEM, TDSE_ECUDA. */
+int tdse_set_frame_stream(tdse_ctx* ctx, double* frames_host, int capacity, int ring_slots, int include_t0);
+
+/* Wait until every frame sampled so far has landed in the host buffer of tdse_set_frame_stream; *nframes = frames kept per
+ * entry.  Errors: TDSE_ESTATE if the streamed mode is off. */
+int tdse_frames_sync(tdse_ctx* ctx, int* nframes);
+
 /* Pairwise dissimilarity of the batch entries' trajectories, eq (16) PAPER.md:219-221:
  *   d_kj = 1/(t1-t0) int_{t0}^{t1} ( int_D (rho_k - rho_j)^2 dr )^{1/2} dt
  * evaluated as the mean over frames first_frame .. last_frame (inclusive) of sqrt(dx^2 * sum over the plane of

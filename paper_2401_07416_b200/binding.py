@@ -30,7 +30,7 @@ SYMBOLS = [
     "tdse_set_wavepacket", "tdse_set_state", "tdse_set_detector", "tdse_step",
     "tdse_detector_read", "tdse_detector_device", "tdse_read_psi", "tdse_read_potential",
     "tdse_norm", "tdse_set_option", "tdse_get_info", "tdse_last_error",
-    "tdse_set_frames", "tdse_frames_read", "tdse_frames_device", "tdse_dissimilarity", "tdse_set_spacing", "tdse_set_potential_cell", "tdse_set_potential_batch",
+    "tdse_set_frames", "tdse_frames_read", "tdse_frames_device", "tdse_dissimilarity", "tdse_set_spacing", "tdse_set_potential_cell", "tdse_set_potential_batch", "tdse_set_frame_stream", "tdse_frames_sync",
 ]
 
 
@@ -78,6 +78,8 @@ def load():
     L.tdse_set_frames.argtypes = [vp, C.c_int, C.c_int]
     L.tdse_frames_read.argtypes = [vp, C.c_int, C.c_int, C.c_int, dp, ip]
     L.tdse_frames_device.argtypes = [vp, C.POINTER(vp), ip, ip]
+    L.tdse_set_frame_stream.argtypes = [vp, dp, C.c_int, C.c_int, C.c_int]
+    L.tdse_frames_sync.argtypes = [vp, ip]
     L.tdse_dissimilarity.argtypes = [vp, C.c_int, C.c_int, dp]
     L.tdse_read_psi.argtypes = [vp, C.c_int, vp, vp]
     L.tdse_read_potential.argtypes = [vp, C.c_int, vp]
@@ -136,8 +138,9 @@ class Tdse:
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h:
-            self.L.tdse_destroy(self._h)
+            self.L.tdse_destroy(self._h)     # synchronises both streams: the host frame buffer may go afterwards
             self._h = C.c_void_p()
+            self._frames_host = None
 
     def __del__(self):
         try:
@@ -239,6 +242,23 @@ class Tdse:
         self._check(self.L.tdse_frames_read(self._h, b, int(first), int(count), out.ctypes.data_as(C.POINTER(C.c_double)),
                                             C.byref(n)), "tdse_frames_read")
         return out
+
+    def set_frame_stream(self, capacity, ring_slots=4, include_t0=True, pinned=True):
+        """Streamed frame mode: torch owns the (page-locked) host buffer [batch][capacity][ny][nx]; the library fills it."""
+        torch = self._torch
+        self._frames_host = None
+        if capacity > 0:
+            buf = torch.empty((self.batch, int(capacity), self.ny, self.nx), dtype=torch.float64)
+            self._frames_host = buf.pin_memory() if pinned else buf
+        ptr = C.cast(self._frames_host.data_ptr(), C.POINTER(C.c_double)) if capacity > 0 else None
+        self._check(self.L.tdse_set_frame_stream(self._h, ptr, int(capacity), int(ring_slots), 1 if include_t0 else 0),
+                    "tdse_set_frame_stream")
+
+    def frames_sync(self) -> np.ndarray:
+        """Frames landed so far as a numpy view [batch][nframes][ny][nx] of the host buffer."""
+        n = C.c_int(0)
+        self._check(self.L.tdse_frames_sync(self._h, C.byref(n)), "tdse_frames_sync")
+        return self._frames_host.numpy()[:, : n.value]
 
     def dissimilarity(self, first_frame, last_frame) -> np.ndarray:
         d = np.empty((self.batch, self.batch), dtype=np.float64)

@@ -76,6 +76,14 @@ struct tdse_ctx {
     int k_det = 0, every = 0, max_samples = 0, nsamples = 0;
     double* frames = nullptr;           // frame mode: [batch][max_frames][ny][nx]
     int max_frames = 0, nframes = 0, frames_t0 = 1;
+    // streamed frame mode (tdse_set_frame_stream): a device ring of fs_slots sample slots [slot][batch][ny][nx]; every
+    // finished slot leaves on a second stream into the caller's host buffer [batch][fs_capacity][ny][nx]
+    double* fs_ring = nullptr;
+    double* fs_host = nullptr;
+    int fs_slots = 0, fs_capacity = 0;
+    cudaStream_t fs_stream = nullptr;
+    std::vector<cudaEvent_t> fs_written, fs_copied;
+    std::vector<char> fs_busy;          // fs_copied[slot] has been recorded since the last reset
     long long steps = 0;
     std::vector<char> have_V, have_state;
     double vabs_max = 0.0;
@@ -204,7 +212,7 @@ int reset_detector(tdse_ctx* c)
 {
     c->steps = 0;
     c->nsamples = 0;
-    c->nframes = 0;
+    c->nframes = 0;                      // streamed mode: frame 0 again; copies still in flight stay ordered on fs_stream
     if (c->D) {
         const long long n = (long long)c->g.batch * c->g.plane;
         fill_zero_kernel<<<(unsigned)std::min<long long>((n + 255) / 256, 4096), 256, 0, c->stream>>>(c->D, n);
@@ -475,9 +483,51 @@ int launch_twopass_step(tdse_ctx* c)
     return TDSE_OK;
 }
 
+// Streamed frame mode: the ring slot the next frame goes to (NULL once the host buffer is full).  The compute stream first
+// waits until the copy that last used this slot has left it.
+int stream_frame_begin(tdse_ctx* c, double** frame)
+{
+    *frame = nullptr;
+    if (c->nframes >= c->fs_capacity) return TDSE_OK;
+    const int slot = c->nframes % c->fs_slots;
+    if (c->fs_busy[slot]) CU_TRY(c, cudaStreamWaitEvent(c->stream, c->fs_copied[slot], 0));
+    *frame = c->fs_ring + (size_t)slot * c->g.batch * c->g.plane;
+    return TDSE_OK;
+}
+
+// ... and its way out: once the detector kernel has written the slot, one strided copy on the second stream puts entry b's
+// frame at frames_host[(b * capacity + nframes) * ny * nx] (one cudaMemcpy2DAsync per slot: rows = entries).
+int stream_frame_end(tdse_ctx* c, double* frame)
+{
+    if (frame) {
+        const int slot = c->nframes % c->fs_slots;
+        const size_t plane_bytes = (size_t)c->g.plane * sizeof(double);
+        CU_TRY(c, cudaEventRecord(c->fs_written[slot], c->stream));
+        CU_TRY(c, cudaStreamWaitEvent(c->fs_stream, c->fs_written[slot], 0));
+        CU_TRY(c, cudaMemcpy2DAsync(c->fs_host + (size_t)c->nframes * c->g.plane, (size_t)c->fs_capacity * plane_bytes, frame, plane_bytes,
+                                    plane_bytes, (size_t)c->g.batch, cudaMemcpyDeviceToHost, c->fs_stream));
+        CU_TRY(c, cudaEventRecord(c->fs_copied[slot], c->fs_stream));
+        c->fs_busy[slot] = 1;
+    }
+    c->nframes++;
+    return TDSE_OK;
+}
+
+void free_frame_stream(tdse_ctx* c)
+{
+    if (c->fs_stream) cudaStreamSynchronize(c->fs_stream);
+    if (c->fs_ring) cudaFree(c->fs_ring);
+    for (cudaEvent_t e : c->fs_written) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->fs_copied) cudaEventDestroy(e);
+    if (c->fs_stream) cudaStreamDestroy(c->fs_stream);
+    c->fs_ring = nullptr; c->fs_host = nullptr; c->fs_stream = nullptr;
+    c->fs_written.clear(); c->fs_copied.clear(); c->fs_busy.clear();
+    c->fs_slots = c->fs_capacity = 0;
+}
+
 // one launch per sample (accumulate + trace), programmatically serialised behind the step kernel
 template <typename real>
-int launch_detector(tdse_ctx* c, double* D, double* partial, double* frame, int slot)
+int launch_detector(tdse_ctx* c, double* D, double* partial, double* frame, long long frame_entry_stride, int slot)
 {
     const unsigned nblk = (unsigned)((c->g.plane + 255) / 256);
     cudaLaunchConfig_t lc = {};
@@ -487,7 +537,7 @@ int launch_detector(tdse_ctx* c, double* D, double* partial, double* frame, int 
     la[0].val.programmaticStreamSerializationAllowed = c->opt_pdl ? 1 : 0;
     lc.attrs = la; lc.numAttrs = 1;
     CU_TRY(c, cudaLaunchKernelEx(&lc, detector_accum_kernel<real>, c->g, c->k_det, static_cast<const real*>(c->R[c->cur]),
-                                 static_cast<const real*>(c->I[c->cur]), D, partial, frame, (long long)c->max_frames * c->g.plane,
+                                 static_cast<const real*>(c->I[c->cur]), D, partial, frame, frame_entry_stride,
                                  c->done, c->m.dx * c->m.dy, c->trace, c->max_samples, slot));
     c->launches++;
     return TDSE_OK;
@@ -503,10 +553,19 @@ int sample_detector(tdse_ctx* c)
         CU_TRY(c, cudaMalloc(&c->done, (size_t)c->g.batch * sizeof(unsigned)));
         CU_TRY(c, cudaMemsetAsync(c->done, 0, (size_t)c->g.batch * sizeof(unsigned), c->stream));
     }
-    double* frame = (c->frames && c->nframes < c->max_frames) ? c->frames + (size_t)c->nframes * c->g.plane : nullptr;
-    rc = launch_detector<real>(c, c->D, c->partial, frame, c->nsamples);
-    if (rc) return rc;
-    if (c->frames) c->nframes++;
+    if (c->fs_ring) {
+        double* frame = nullptr;
+        rc = stream_frame_begin(c, &frame);
+        if (rc) return rc;
+        rc = launch_detector<real>(c, c->D, c->partial, frame, c->g.plane, c->nsamples);
+        if (rc) return rc;
+        if ((rc = stream_frame_end(c, frame))) return rc;
+    } else {
+        double* frame = (c->frames && c->nframes < c->max_frames) ? c->frames + (size_t)c->nframes * c->g.plane : nullptr;
+        rc = launch_detector<real>(c, c->D, c->partial, frame, (long long)c->max_frames * c->g.plane, c->nsamples);
+        if (rc) return rc;
+        if (c->frames) c->nframes++;
+    }
     c->nsamples++;
     return TDSE_OK;
 }
@@ -515,7 +574,14 @@ int sample_detector(tdse_ctx* c)
 template <typename real>
 int sample_initial_frame(tdse_ctx* c)
 {
-    const int rc = launch_detector<real>(c, nullptr, nullptr, c->frames, 0);
+    if (c->fs_ring) {
+        double* frame = nullptr;
+        int rc = stream_frame_begin(c, &frame);
+        if (rc) return rc;
+        if ((rc = launch_detector<real>(c, nullptr, nullptr, frame, c->g.plane, 0))) return rc;
+        return stream_frame_end(c, frame);
+    }
+    const int rc = launch_detector<real>(c, nullptr, nullptr, c->frames, (long long)c->max_frames * c->g.plane, 0);
     if (rc) return rc;
     c->nframes = 1;
     return TDSE_OK;
@@ -596,6 +662,7 @@ int tdse_destroy(tdse_ctx* c)
     if (c->D) cudaFree(c->D);
     if (c->trace) cudaFree(c->trace);
     if (c->frames) cudaFree(c->frames);
+    free_frame_stream(c);
     if (c->partial) cudaFree(c->partial);
     if (c->done) cudaFree(c->done);
     if (c->scalars) cudaFree(c->scalars);
@@ -1027,7 +1094,7 @@ int tdse_step(tdse_ctx* c, int n)
         return fail(c, TDSE_EINVAL, "tdse_step: fused kernel needs a 5-array workspace, rows of whole 16-byte groups, even ny, nx >= 8 and ny >= 8");
     const int tmax = (c->opt_tblock > 0) ? c->opt_tblock : (kernel == TDSE_KERNEL_FUSED ? auto_tblock(c) : 1);
     c->last_kernel = kernel;
-    if (n > 0 && c->frames && c->frames_t0 && c->every > 0 && c->steps == 0 && c->nframes == 0) {
+    if (n > 0 && (c->frames || c->fs_ring) && c->frames_t0 && c->every > 0 && c->steps == 0 && c->nframes == 0) {
         const int rc0 = (c->dtype == TDSE_F32) ? sample_initial_frame<float>(c) : sample_initial_frame<double>(c);
         if (rc0) return rc0;
     }
@@ -1090,6 +1157,7 @@ int tdse_set_frames(tdse_ctx* c, int max_frames, int include_t0)
     DeviceScope on_device_(c);
     if (max_frames < 0) return fail(c, TDSE_EINVAL, "tdse_set_frames: max_frames < 0");
     CU_TRY(c, cudaStreamSynchronize(c->stream));
+    free_frame_stream(c);                // flat and streamed frame mode exclude each other
     if (c->frames) { cudaFree(c->frames); c->frames = nullptr; }
     c->max_frames = 0; c->frames_t0 = include_t0 ? 1 : 0;
     if (max_frames > 0) {
@@ -1123,6 +1191,45 @@ int tdse_frames_device(tdse_ctx* c, double** frames_device, int* max_frames, int
     if (frames_device) *frames_device = c->frames;
     if (max_frames) *max_frames = c->max_frames;
     if (nframes) *nframes = c->nframes;
+    return TDSE_OK;
+}
+
+int tdse_set_frame_stream(tdse_ctx* c, double* frames_host, int capacity, int ring_slots, int include_t0)
+{
+    if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
+    if (capacity < 0 || ring_slots < 0) return fail(c, TDSE_EINVAL, "tdse_set_frame_stream: capacity, ring_slots must be >= 0");
+    if (capacity > 0 && (!frames_host || ring_slots < 2)) return fail(c, TDSE_EINVAL, "tdse_set_frame_stream: needs a host buffer and at least 2 ring slots");
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    free_frame_stream(c);
+    if (c->frames) { cudaFree(c->frames); c->frames = nullptr; c->max_frames = 0; }
+    c->frames_t0 = include_t0 ? 1 : 0;
+    if (capacity > 0) {
+        ring_slots = std::min(ring_slots, capacity);
+        cudaError_t e = cudaMalloc(&c->fs_ring, (size_t)ring_slots * c->g.batch * c->g.plane * sizeof(double));
+        if (e != cudaSuccess) { cudaGetLastError(); c->fs_ring = nullptr; return fail(c, TDSE_ENOMEM, std::string("tdse_set_frame_stream: ring: ") + cudaGetErrorString(e)); }
+        if ((e = cudaStreamCreateWithFlags(&c->fs_stream, cudaStreamNonBlocking)) != cudaSuccess) { free_frame_stream(c); return fail(c, TDSE_ECUDA, "tdse_set_frame_stream: stream"); }
+        c->fs_written.assign(ring_slots, nullptr); c->fs_copied.assign(ring_slots, nullptr); c->fs_busy.assign(ring_slots, 0);
+        for (int q = 0; q < ring_slots; ++q) {
+            if (cudaEventCreateWithFlags(&c->fs_written[q], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&c->fs_copied[q], cudaEventDisableTiming) != cudaSuccess) {
+                free_frame_stream(c);
+                return fail(c, TDSE_ECUDA, "tdse_set_frame_stream: events");
+            }
+        }
+        c->fs_host = frames_host; c->fs_slots = ring_slots; c->fs_capacity = capacity;
+    }
+    return reset_detector(c);
+}
+
+int tdse_frames_sync(tdse_ctx* c, int* nframes)
+{
+    if (!c) return TDSE_EINVAL;
+    DeviceScope on_device_(c);
+    if (!c->fs_ring) return fail(c, TDSE_ESTATE, "tdse_frames_sync: streamed frame mode is off (tdse_set_frame_stream)");
+    CU_TRY(c, cudaStreamSynchronize(c->stream));       // every sample has been launched and has handed its slot over ...
+    CU_TRY(c, cudaStreamSynchronize(c->fs_stream));    // ... and every copy has landed
+    if (nframes) *nframes = std::min(c->nframes, c->fs_capacity);
     return TDSE_OK;
 }
 

@@ -72,7 +72,7 @@ __device__ __forceinline__ double axis_gap(double a, double lo, double hi, doubl
 
 // A block owns a brick of kPotBX x kPotBY x kPotBZ threads = (CELLS kPotBX) x kPotBY x kPotBZ cells of entry blockIdx.y.
 // HAS_CUT: atoms farther than rcut from every cell of the brick are dropped while the list is staged (ordered
-// compaction, so the summation order of the kept atoms is the list order); the pair test itself is the oracle's.
+// compaction, so the summation order of the kept atoms is the list order); the pair test itself is that of the definition (include/tdse.h).
 // PREFIX_OUT: write the unclamped fp64 sums to `prefix_out` (flat [nz][ny][nx]) instead of V.
 constexpr int kPotBX = 16, kPotBY = 4, kPotBZ = 4;
 

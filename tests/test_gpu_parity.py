@@ -908,3 +908,47 @@ def test_iteration_barrier_variants_are_bit_identical(tblock, dtype, shape, bc, 
         for b in range(batch):
             for x0, x1 in zip(out[0][b], res[b]):
                 assert np.array_equal(x0, x1), "variant %d, entry %d" % (v, b)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("include_t0,ring_slots,pinned", [(True, 2, True), (False, 3, True), (True, 5, False)])
+def test_streamed_frames_equal_the_flat_frame_mode_bit_for_bit(dtype, include_t0, ring_slots, pinned):
+    """tdse_set_frame_stream (device ring of a few sample slots, one asynchronous copy per slot into a host buffer) keeps
+    the frames tdse_set_frames keeps, every bit, with many more frames than ring slots; the accumulated image and the trace
+    do not change; frames beyond the capacity are dropped; and a second trajectory after a reset starts at frame 0 again."""
+    from paper_2401_07416_b200 import Tdse, TdseError, TDSE_ESTATE
+    w = make_config(3, n=(40, 36, 44), batch=3, steps=57, dtype=dtype).with_(every=3)
+    nfr = w.steps // w.every + (1 if include_t0 else 0)
+    flat = Tdse.from_workload(w)
+    flat.set_frames(nfr, include_t0)
+    flat.step(w.steps)
+    want = [flat.frames_read(b) for b in range(w.batch)]
+    want_det = [flat.detector_read(b) for b in range(w.batch)]
+    flat.close()
+
+    t = Tdse.from_workload(w)
+    with pytest.raises(TdseError) as e:
+        t.frames_sync()
+    assert e.value.code == TDSE_ESTATE
+    cap = nfr - 2                                          # the last two frames do not fit
+    t.set_frame_stream(cap, ring_slots, include_t0, pinned=pinned)
+    t.step(20)
+    t.step(w.steps - 20)
+    got = t.frames_sync()
+    assert got.shape == (w.batch, cap, w.ny, w.nx) and t.get_info("nframes") == nfr
+    for b in range(w.batch):
+        assert np.array_equal(got[b], want[b][:cap])
+        D, tr = t.detector_read(b)
+        assert np.array_equal(D, want_det[b][0]) and np.array_equal(tr, want_det[b][1])
+    with pytest.raises(TdseError) as e:                    # the frames are not on the device in this mode
+        t.dissimilarity(0, 1)
+    assert e.value.code == TDSE_ESTATE
+    # a second trajectory: same packet again, frames restart at slot 0
+    p = w.packet
+    t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
+    t.step(w.steps)
+    again = t.frames_sync()
+    for b in range(w.batch):
+        assert np.array_equal(again[b], want[b][:cap])
+    t.set_frame_stream(0, 0)                               # off
+    t.close()
