@@ -225,8 +225,168 @@ def fp32_vs_fp64_agreement(device):
     return {"grid": [384, 384, 384], "fdtd_steps": int(w.steps), "detector_rel_l2_f32_vs_f64": d}
 
 
+def _gpu_timer(stream):
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    return e0, e1
+
+
+def run_widened(a):
+    """--workload f1|f2|f3: throughput of the rows widened after the step loop, one JSON line each.
+
+    f1  frame-mode detector on the cfg3 workload: step-loop time with frames off / kept on the device / streamed to the host;
+    f2  pairwise trajectory dissimilarity d_kj (eq (16)) over 879 trajectories x 150 frames x 240^2 px
+        (the paper's sample, PAPER.md:211, 221), as GB/s of distinct frame data against the HBM peak;
+    f3  unit-cell potential resampler: a 16 x 16 x 420 cell tiled 15 x 15 onto 240 x 240 x 520, as cells/s and
+        GB/s written against the HBM peak, with the oracle's routine timed beside it (the paper's 15-minute host step).
+    """
+    import torch
+    from paper_2401_07416_b200 import Tdse
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(0)
+    peak, peak_src, _ = peaks()
+    stream = torch.cuda.Stream()
+    reps = max(a.steps, 1)
+    line = {"n_gpus": 1, "steps": reps, "warmup": a.warmup, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "data": "synthetic"}
+
+    if a.workload == "f1":
+        w = make_config(3)
+        if a.nsteps:
+            w = w.with_(steps=a.nsteps)
+        nfr = w.steps // w.every + 1
+        t = Tdse.from_workload(w, stream=stream)
+        p = w.packet
+        res = {}
+        for mode in ("off", "device", "host_stream"):
+            if mode == "device":
+                t.set_frames(nfr, True)
+            elif mode == "host_stream":
+                t.set_frame_stream(nfr, 8, True)
+            best = None
+            for _ in range(a.warmup + reps):
+                t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
+                e0, e1 = _gpu_timer(stream)
+                with torch.cuda.stream(stream):
+                    e0.record(stream); t.step(w.steps); e1.record(stream)
+                if mode == "host_stream":
+                    t.frames_sync()
+                stream.synchronize()
+                ms = e0.elapsed_time(e1)
+                best = ms if best is None else min(best, ms)
+            res[mode] = best
+        t.close()
+        nsamp = w.steps // w.every
+        frame_bytes = w.batch * w.nx * w.ny * 8
+        line.update({"metric": "frame_mode_cost_per_sample", "unit": "us/sample", "dtype": w.dtype,
+                     "value": 1e3 * (res["host_stream"] - res["off"]) / nsamp,
+                     "config": {"workload": "f1: " + w.name, "fdtd_steps": w.steps, "samples": nsamp, "frame_bytes_per_sample": frame_bytes},
+                     "step_loop_ms": res, "us_per_sample_device_frames": 1e3 * (res["device"] - res["off"]) / nsamp,
+                     "us_per_sample_host_stream": 1e3 * (res["host_stream"] - res["off"]) / nsamp,
+                     "higher_is_better": False,
+                     "roofline": {"bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src,
+                                  "achieved": None, "note": "one extra 8-byte store per plane cell and entry per sample (+ its D2H copy over PCIe in host_stream mode)"}})
+        print(json.dumps(line), flush=True)
+        return
+
+    if a.workload == "f2":
+        batch, nfr, n = (a.batch or 879), 150, 240
+        dx = 0.15
+        dt = 0.5 / (6.0 / dx ** 2 + 200.0)
+        t = Tdse(n, n, 8, batch, dx, dt, 1.0, 1.0, "f32", stream=stream)
+        t.set_boundary(0, 0, 1, 0, 0, 0.05, 2)
+        rng = np.random.default_rng(16)
+        lists, off = [], [0]
+        for b in range(batch):     # a few atoms per entry, seeded: every trajectory differs
+            k = 6
+            at = np.stack([rng.uniform(0, n * dx, k), rng.uniform(0, n * dx, k), rng.uniform(0, 8 * dx, k),
+                           np.full(k, 6.0), np.full(k, 0.1), np.full(k, 0.5)], axis=1)
+            lists.append(at); off.append(off[-1] + k)
+        t.set_potential_batch(np.concatenate(lists), off, -200.0, 0.0, 0.0)
+        t.set_wavepacket(-1, n * dx / 2, n * dx / 2, 4 * dx, 4.0, 0.0, 0.0, 3.0, 0.0)
+        t.set_detector(4, 1, 1)
+        t.set_frames(nfr, True)
+        t.step(nfr - 1)
+        assert t.get_info("nframes") == nfr
+        stream.synchronize()
+        best = None
+        for _ in range(a.warmup + reps):
+            t0 = time.perf_counter()
+            d = t.dissimilarity(0, nfr - 1)
+            dt_s = time.perf_counter() - t0
+            best = dt_s if best is None else min(best, dt_s)
+        t.close()
+        distinct = batch * nfr * n * n * 8.0
+        tile = 8
+        tiles = (batch + tile - 1) // tile
+        read = (tiles * (tiles + 1) / 2) * nfr * 2 * tile * n * n * 8.0
+        line.update({"metric": "dissimilarity_distinct_frame_gbs", "unit": "GB/s", "dtype": "f64", "value": distinct / best / 1e9,
+                     "ms_per_step": 1e3 * best,
+                     "config": {"workload": "f2: d_kj of eq (16) over %d trajectories x %d frames x %dx%d px" % (batch, nfr, n, n),
+                                "pairs": batch * (batch - 1) // 2, "distinct_frame_bytes": distinct,
+                                "pair_tile": [tile, tile], "frame_reads_issued_bytes": read, "reuse": "each frame read serves %d pairs" % tile},
+                     "pairs_per_s": batch * (batch - 1) / 2 / best, "d_checksum": float(d.sum()),
+                     "roofline": {"bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src,
+                                  "achieved": read / best / 1e9, "frac": read / best / 1e9 / peak,
+                                  "note": "achieved = frame bytes the blocks read (L2 + DRAM) / time; distinct frame data / time is `value`"}})
+        print(json.dumps(line), flush=True)
+        return
+
+    if a.workload == "f3":
+        nx, ny, nz = 240, 240, 520
+        mx, my, mz = 16, 16, 420
+        A = 0.529177                                   # bohr per Angstrom^-1 ... the paper's mesh: 35.4/240 x 40.9/240 x 70/420 Angstrom
+        dx, dy, dz = 35.4 / 240 / A, 40.9 / 240 / A, 70.0 / 420 / A
+        ax, ay, az = 16 * dx, 16 * dy, (mz - 1) * dz
+        rng = np.random.default_rng(17)
+        cell = -rng.uniform(0.0, 10.0, (mz, my, mx))
+        dt = 0.2 * min(dx, dy, dz) ** 2
+        batch = a.batch or 8
+        t = Tdse(nx, ny, nz, batch, dx, dt, 1.0, 1.0, "f32", stream=stream)
+        t.set_spacing(dy, dz)
+        t.set_boundary(0, 0, 0, 0, 32, 0.05, 2)
+        cell_dev = torch.from_numpy(cell).cuda()
+        torch.cuda.synchronize()
+        best = None
+        for _ in range(a.warmup + reps):
+            e0, e1 = _gpu_timer(stream)
+            with torch.cuda.stream(stream):
+                e0.record(stream)
+                for b in range(batch):
+                    t.set_potential_cell(b, cell_dev, (ax, ay, az), (0.0, 0.0, 2.0), -50.0, 0.0)
+                e1.record(stream)
+            stream.synchronize()
+            ms = e0.elapsed_time(e1)
+            best = ms if best is None else min(best, ms)
+        V0 = t.read_potential(0)
+        t.close()
+        import oracle
+        oracle.set_threads(len(os.sched_getaffinity(0)))
+        t0 = time.perf_counter()
+        Vo = oracle.potential_cell(nx, ny, nz, dx, cell, (ax, ay, az), (0.0, 0.0, 2.0), -50.0, 0.0, dy, dz)
+        cpu_s = time.perf_counter() - t0
+        err = float(np.max(np.abs(V0.astype(np.float64) - Vo.astype(np.float32).astype(np.float64))))
+        cells = float(nx) * ny * nz * batch
+        wbytes = (nx + 8.0) * (ny + 8.0) * nz * 4 * batch
+        line.update({"metric": "potential_resample_gcells_per_s", "unit": "Gcell/s", "dtype": "f32", "value": cells / (best * 1e-3) / 1e9,
+                     "ms_per_step": best,
+                     "config": {"workload": "f3: %dx%dx%d unit cell tiled 15x15 onto %dx%dx%d, %d entries" % (mx, my, mz, nx, ny, nz, batch)},
+                     "max_abs_diff_vs_oracle_entry0": err,
+                     "roofline": {"bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src,
+                                  "achieved": wbytes / (best * 1e-3) / 1e9, "frac": wbytes / (best * 1e-3) / 1e9 / peak,
+                                  "note": "bytes written (framed V, 4 B per stored cell); the 861 KB unit cell is read from L2"},
+                     "cpu_baseline": {"value": float(nx) * ny * nz / cpu_s / 1e9, "unit": "Gcell/s", "cores": oracle.max_threads(),
+                                      "kind": "oracle", "sample": "one entry, oracle_potential_cell as it stands (%.2f s)" % cpu_s}})
+        print(json.dumps(line), flush=True)
+        return
+    raise SystemExit("unknown workload " + a.workload)
+
+
 def main():
     a = parse_args()
+    if a.workload in ("f1", "f2", "f3"):
+        return run_widened(a)
     if a.impl == "reference":
         return run_reference(a)
 

@@ -397,26 +397,30 @@ bool want_split(tdse_ctx* c)
     return (long long)tx * ty * nch * c->g.batch <= c->num_sms;
 }
 
+// default prefetch depth: the launcher picks the barrier scheme (SPLIT)
+template <typename real, int T, int BX, int BY, int NT, int PF, bool GHOSTXY>
+int launch_fused_default(tdse_ctx* c, FusedParams& P)
+{
+    return want_split<real, T, BX, BY, NT, PF>(c) ? launch_fused_cfg<real, T, BX, BY, NT, PF, GHOSTXY, 1, true>(c, P, 1)
+                                                  : launch_fused_cfg<real, T, BX, BY, NT, PF, GHOSTXY, 1, false>(c, P, 1);
+}
+
 template <bool GHOSTXY>
 int launch_fused_bc(tdse_ctx* c, FusedParams& P, int T)
 {
     if (c->dtype == TDSE_F32) {
         if (T == 2) return c->opt_pf == 1 ? launch_fused_cfg<float, 2, 64, 32, 384, 1, GHOSTXY>(c, P, 1)
-                         : want_split<float, 2, 64, 32, 384, 2>(c) ? launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY, 1, true>(c, P, 1)
-                                                                   : launch_fused_cfg<float, 2, 64, 32, 384, 2, GHOSTXY>(c, P, 1);
+                                          : launch_fused_default<float, 2, 64, 32, 384, 2, GHOSTXY>(c, P);
         return c->opt_pf == 1 ? launch_fused_cfg<float, 1, 64, 32, 352, 1, GHOSTXY>(c, P, 1)
              : c->opt_pf == 2 ? launch_fused_cfg<float, 1, 64, 32, 352, 2, GHOSTXY>(c, P, 1)
-             : want_split<float, 1, 64, 32, 352, 4>(c) ? launch_fused_cfg<float, 1, 64, 32, 352, 4, GHOSTXY, 1, true>(c, P, 1)
-                                                       : launch_fused_cfg<float, 1, 64, 32, 352, 4, GHOSTXY>(c, P, 1);
+                              : launch_fused_default<float, 1, 64, 32, 352, 4, GHOSTXY>(c, P);
     }
     if (T == 2) return c->opt_pf == 1 ? launch_fused_cfg<double, 2, 32, 24, 320, 1, GHOSTXY>(c, P, 1)
                      : c->opt_pf == 2 ? launch_fused_cfg<double, 2, 32, 24, 320, 2, GHOSTXY>(c, P, 1)
-                     : want_split<double, 2, 32, 24, 320, 3>(c) ? launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY, 1, true>(c, P, 1)
-                                                                : launch_fused_cfg<double, 2, 32, 24, 320, 3, GHOSTXY>(c, P, 1);
+                                      : launch_fused_default<double, 2, 32, 24, 320, 3, GHOSTXY>(c, P);
     return c->opt_pf == 1 ? launch_fused_cfg<double, 1, 32, 32, 352, 1, GHOSTXY>(c, P, 1)
          : c->opt_pf == 2 ? launch_fused_cfg<double, 1, 32, 32, 352, 2, GHOSTXY>(c, P, 1)
-         : want_split<double, 1, 32, 32, 352, 4>(c) ? launch_fused_cfg<double, 1, 32, 32, 352, 4, GHOSTXY, 1, true>(c, P, 1)
-                                                    : launch_fused_cfg<double, 1, 32, 32, 352, 4, GHOSTXY>(c, P, 1);
+                          : launch_fused_default<double, 1, 32, 32, 352, 4, GHOSTXY>(c, P);
 }
 
 int launch_fused(tdse_ctx* c, FusedParams& P, int T)
@@ -1011,16 +1015,15 @@ int tdse_set_wavepacket(tdse_ctx* c, int b, double x0, double y0, double z0, dou
     p.kx = kx; p.ky = ky; p.kz = kz;
     p.amp = amplitude != 0.0 ? amplitude : std::pow(pi * sigma * sigma, -0.75);
     const unsigned nblk = (unsigned)((c->g.cells + 255) / 256);
-    for (int e = b0; e < b1; ++e) {
-        if (c->dtype == TDSE_F32)
-            wavepacket_init_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->m, p,
-                (const float*)entry_ptr(c, c->V, e), (float*)entry_ptr(c, c->R[c->cur], e), (float*)entry_ptr(c, c->I[c->cur], e));
-        else
-            wavepacket_init_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->m, p,
-                (const double*)entry_ptr(c, c->V, e), (double*)entry_ptr(c, c->R[c->cur], e), (double*)entry_ptr(c, c->I[c->cur], e));
-        CU_LAUNCH_CHECK(c);
-        c->have_state[e] = 1;
-    }
+    // one launch for all the entries that get this packet: a thread evaluates it once and walks the entries
+    if (c->dtype == TDSE_F32)
+        wavepacket_init_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->m, p, b1 - b0,
+            (const float*)entry_ptr(c, c->V, b0), (float*)entry_ptr(c, c->R[c->cur], b0), (float*)entry_ptr(c, c->I[c->cur], b0));
+    else
+        wavepacket_init_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->m, p, b1 - b0,
+            (const double*)entry_ptr(c, c->V, b0), (double*)entry_ptr(c, c->R[c->cur], b0), (double*)entry_ptr(c, c->I[c->cur], b0));
+    CU_LAUNCH_CHECK(c);
+    for (int e = b0; e < b1; ++e) c->have_state[e] = 1;
     return reset_detector(c);
 }
 

@@ -14,8 +14,8 @@ struct AtomRec { double x, y, z, Z, soft2, screen; };   // same layout as tdse_a
 //   * a thread owns CELLS consecutive cells along x and shares the y/z part of the distance among them;
 //   * atoms are staged through shared memory in chunks with 1/lambda precomputed;
 //   * inverse square roots: the hardware seed (MUFU.RSQ64H through rsqrt.approx.ftz.f64) + one third-order step;
-//   * exp(-r/lambda): x = n ln2/32 + r, exp(x) = 2^(n div 32) * T[n mod 32] * (1 + q(r)), T[j] = 2^(j/32) in shared
-//     memory, q = expm1 as a degree-6 polynomial on |r| <= ln2/64 (remainder < 4e-18);
+//   * exp(-r/lambda): x = n ln2/128 + r, exp(x) = 2^(n div 128) * T[n mod 128] * (1 + q(r)), T[j] = 2^(j/128) in shared
+//     memory, q = expm1 as a degree-5 polynomial on |r| <= ln2/256 (remainder < 6e-19);
 //   * nearest image by the round-to-nearest-even magic constant instead of rint.
 // Double accumulate in list order, one rounding to `real`.  One launch covers every batch entry (blockIdx.y); the
 // sum may start from a per-cell prefix (the atoms all entries share, summed once: prefix_out mode) -- the same sequence of
@@ -39,23 +39,25 @@ __device__ __forceinline__ double rsqrt_pos(double a)
     return fma(y * e, p, y);
 }
 
-// exp(x) for -30000 < x <= 0 with the 2^(j/32) table `T` (shared memory); below -708 the result stays near 2^-1022, which
-// no sum registers.  exp(-0) = 1 exactly.
+// exp(x) for -30000 < x <= 0 with the 2^(j/128) table `T` (shared memory): x = n ln2/128 + r, |r| <= ln2/256, and
+// exp(x) = 2^(n div 128) * T[n mod 128] * (1 + q(r)), q = expm1 as a degree-5 polynomial (remainder r^6/720 < 6e-19).
+// r comes from one fma with ln2/128 rounded to double: its error, |n| * 2^-60, stays below 2e-15 for every term that
+// is not itself below 1e-16 (|x| < 37).  Below x = -708 the result stays near 2^-1022, which no sum registers.  exp(-0) = 1.
+constexpr int kExpTable = 128;
+
 __device__ __forceinline__ double exp_nonpositive(double x, const double* __restrict__ T)
 {
-    double t = fma(x, 32.0 * 1.4426950408889634074, kRoundMagic);
-    const int n = max(__double2loint(t), -1022 * 32);               // n = 32 k + j; k >= -1022 keeps the result a normal number
+    double t = fma(x, (double)kExpTable * 1.4426950408889634074, kRoundMagic);
+    const int n = max(__double2loint(t), -1022 * kExpTable);        // n = 128 k + j; k >= -1022 keeps the result a normal number
     t -= kRoundMagic;
-    double r = fma(t, -6.93147180369123816490e-01 / 32.0, x);       // ln2 hi (32 significant bits: t * hi is exact)
-    r = fma(t, -1.90821492927058770002e-10 / 32.0, r);              // |r| <= ln2 / 64
-    double p = fma(r, 1.0 / 720.0, 1.0 / 120.0);
-    p = fma(p, r, 1.0 / 24.0);
+    const double r = fma(t, -0.69314718055994530942 / (double)kExpTable, x);
+    double p = fma(r, 1.0 / 120.0, 1.0 / 24.0);
     p = fma(p, r, 1.0 / 6.0);
     p = fma(p, r, 0.5);
     p = fma(p, r, 1.0);
-    const double s = T[n & 31];
-    const double v = fma(s, p * r, s);                              // 2^(j/32) e^r in [0.5, 2)
-    return __hiloint2double(__double2hiint(v) + ((n >> 5) << 20), __double2loint(v));   // * 2^k, k >= -1022
+    const double s = T[n & (kExpTable - 1)];
+    const double v = fma(s, p * r, s);                              // 2^(j/128) e^r in [0.5, 2)
+    return __hiloint2double(__double2hiint(v) + ((n >> 7) << 20), __double2loint(v));   // * 2^k
 }
 
 // distance from coordinate a to the interval [lo, hi] along one axis (nearest periodic image if L > 0)
@@ -77,7 +79,7 @@ __device__ __forceinline__ double axis_gap(double a, double lo, double hi, doubl
 constexpr int kPotBX = 16, kPotBY = 4, kPotBZ = 4;
 
 template <typename real, int CELLS, bool HAS_CUT, bool PREFIX_OUT>
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(256, 3)
 potential_build_kernel(Grid g, double dx, double dy, double dz, const AtomRec* __restrict__ atoms,
                        const AtomRange* __restrict__ ranges /* [gridDim.y] or NULL */, int first0, int count0,
                        const double* __restrict__ prefix_in /* flat fp64 sums of the atoms before `first`, or NULL */,
@@ -86,7 +88,7 @@ potential_build_kernel(Grid g, double dx, double dy, double dz, const AtomRec* _
 {
     static_assert(kPotBX * kPotBY * kPotBZ == 256 && kAtomChunk <= 256, "block shape");
     __shared__ AtomStaged s_atoms[kAtomChunk];
-    __shared__ double s_exp2[32];
+    __shared__ double s_exp2[kExpTable];
     __shared__ int s_warp_count[8];
     const int tx = threadIdx.x % kPotBX, ty = (threadIdx.x / kPotBX) % kPotBY, tz = threadIdx.x / (kPotBX * kPotBY);
     const int bricks_x = (g.nx + CELLS * kPotBX - 1) / (CELLS * kPotBX), bricks_y = (g.ny + kPotBY - 1) / kPotBY;
@@ -104,7 +106,8 @@ potential_build_kernel(Grid g, double dx, double dy, double dz, const AtomRec* _
     const double lox = (bx * kPotBX * CELLS - 1) * dx, hix = ((bx + 1) * kPotBX * CELLS) * dx;
     const double loy = (by * kPotBY - 1) * dy, hiy = ((by + 1) * kPotBY) * dy;
     const double loz = (bz * kPotBZ - 1) * dz, hiz = ((bz + 1) * kPotBZ) * dz;
-    if (threadIdx.x < 32) s_exp2[threadIdx.x] = exp2((double)threadIdx.x / 32.0);
+    static_assert(kExpTable == 128, "n >> 7 above");
+    if (threadIdx.x < kExpTable) s_exp2[threadIdx.x] = exp2((double)threadIdx.x / (double)kExpTable);
     double sum[CELLS], xs[CELLS];
 #pragma unroll
     for (int e = 0; e < CELLS; ++e) xs[e] = (i0 + e) * dx;
@@ -211,9 +214,9 @@ potential_cell_kernel(Grid g, double dx, double dy, double dz, const double* __r
 {
     const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= g.cells) return;
-    const int i = (int)(c % g.nx);
     const long long t = c / g.nx;
-    const int j = (int)(t % g.ny), k = (int)(t / g.ny);
+    const int i = (int)(c - t * g.nx);
+    const int k = (int)(t / g.ny), j = (int)(t - (long long)k * g.ny);
     const double hx = p.ax / p.mx, hy = p.ay / p.my, hz = (p.mz > 1) ? p.az / (p.mz - 1) : 1.0;
     const double u = (i * dx - p.x0) / hx, v = (j * dy - p.y0) / hy;
     const double w = fmin(fmax((k * dz - p.z0) / hz, 0.0), (double)(p.mz - 1));
@@ -222,10 +225,11 @@ potential_cell_kernel(Grid g, double dx, double dy, double dz, const double* __r
     int iw0 = min((int)floor(w), p.mz > 1 ? p.mz - 2 : 0);
     const double tw = (p.mz > 1) ? w - (double)iw0 : 0.0;
     const int iw1 = (p.mz > 1) ? iw0 + 1 : 0;
-    long long iu0 = (long long)fu % p.mx; if (iu0 < 0) iu0 += p.mx;
-    long long iv0 = (long long)fv % p.my; if (iv0 < 0) iv0 += p.my;
-    const long long iu1 = (iu0 + 1) % p.mx, iv1 = (iv0 + 1) % p.my;
-    auto at = [&](long long a, long long b, int cz) { return cell[((long long)cz * p.my + b) * p.mx + a]; };
+    // periodic cell index of floor(u): fu - mx * floor(fu / mx), exact in double for any mesh (no 64-bit integer division)
+    const int iu0 = (int)(fu - (double)p.mx * floor(fu / (double)p.mx));
+    const int iv0 = (int)(fv - (double)p.my * floor(fv / (double)p.my));
+    const int iu1 = iu0 + 1 == p.mx ? 0 : iu0 + 1, iv1 = iv0 + 1 == p.my ? 0 : iv0 + 1;
+    auto at = [&](int a, int b, int cz) { return __ldg(cell + ((long long)cz * p.my + b) * p.mx + a); };
     // same grouping as the definition: x, then y, then z; products and sums kept separate (no contraction)
     const double c00 = __dadd_rn(__dmul_rn(at(iu0, iv0, iw0), 1.0 - tu), __dmul_rn(at(iu1, iv0, iw0), tu));
     const double c10 = __dadd_rn(__dmul_rn(at(iu0, iv1, iw0), 1.0 - tu), __dmul_rn(at(iu1, iv1, iw0), tu));
@@ -271,7 +275,7 @@ __device__ __forceinline__ double packet_re_nbr(const PacketParams& p, const Gri
 
 template <typename real>
 __global__ void __launch_bounds__(256)
-wavepacket_init_kernel(Grid g, Mesh m, PacketParams p,
+wavepacket_init_kernel(Grid g, Mesh m, PacketParams p, int nent /* entries that get this packet, consecutive */,
                        const real* __restrict__ V, real* __restrict__ R, real* __restrict__ I)
 {
     const long long cell = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -285,9 +289,15 @@ wavepacket_init_kernel(Grid g, Mesh m, PacketParams p,
     const double d2x = packet_re_nbr(p, g, m, i + 1, j, k) - 2.0 * re + packet_re_nbr(p, g, m, i - 1, j, k);
     const double d2y = packet_re_nbr(p, g, m, i, j + 1, k) - 2.0 * re + packet_re_nbr(p, g, m, i, j - 1, k);
     const double d2z = packet_re_nbr(p, g, m, i, j, k + 1) - 2.0 * re + packet_re_nbr(p, g, m, i, j, k - 1);
-    const double Ar = -m.cx * d2x - m.cy * d2y - m.cz * d2z + m.cv * (double)V[cell_offset(g, i, j, k)] * re;
-    store_with_images(R, g, i, j, k, (real)re);
-    store_with_images(I, g, i, j, k, (real)(im + 0.5 * Ar));
+    const double kin = -m.cx * d2x - m.cy * d2y - m.cz * d2z;
+    const long long o = cell_offset(g, i, j, k);
+    // the packet is the same for every entry; only the potential term of the staggered start differs
+    for (int e = 0; e < nent; ++e) {
+        const long long eo = (long long)e * g.pcells;
+        const double Ar = kin + m.cv * (double)V[eo + o] * re;
+        store_with_images(R + eo, g, i, j, k, (real)re);
+        store_with_images(I + eo, g, i, j, k, (real)(im + 0.5 * Ar));
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -410,10 +420,10 @@ detector_accum_kernel(Grid g, int k_det, const real* __restrict__ R, const real*
 // Trajectory dissimilarity, eq (16), over the batch entries of one context:
 //   d_kj = mean over frames s0..s1 of sqrt( dA * sum_p (rho_k[s][p] - rho_j[s][p])^2 )      (reading 23)
 // A block takes a kDisTile x kDisTile tile of entry pairs and one frame, so every frame it reads serves
-// kDisTile pairs; fixed-order block sums (deterministic).  inner[(k*batch + j)*nwin + s-s0] = sqrt(dA * sum).
+// kDisTile pairs (64 fp64 accumulators per thread: 1 flop per byte read, so the pass stays memory-bound); fixed-order block sums (deterministic).  inner[(k*batch + j)*nwin + s-s0] = sqrt(dA * sum).
 // grid: x = tiles_k * tiles_j, y = nwin.
 // ---------------------------------------------------------------------------------------------
-constexpr int kDisTile = 4;
+constexpr int kDisTile = 8;
 
 __global__ void __launch_bounds__(256)
 dissimilarity_inner_kernel(const double* __restrict__ frames, int batch, long long entry_stride, int npix,

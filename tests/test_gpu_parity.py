@@ -494,7 +494,7 @@ def test_flat_offsets_beyond_2_31_elements_per_array():
 @pytest.mark.parametrize("include_t0", [True, False])
 def test_frames_and_dissimilarity_match_oracle(dtype, include_t0):
     from paper_2401_07416_b200 import Tdse, TdseError, TDSE_EINVAL, TDSE_ESTATE
-    w = make_config(3, n=(40, 36, 44), batch=5, steps=46, dtype=dtype)     # 5 entries: a full 4x4 pair tile + a ragged one
+    w = make_config(3, n=(40, 36, 44), batch=10, steps=46, dtype=dtype)    # 10 entries: a full 8x8 pair tile + ragged ones
     w = w.with_(every=5)
     t = Tdse.from_workload(w)
     with pytest.raises(TdseError) as e:                    # frame mode is off
@@ -521,7 +521,7 @@ def test_frames_and_dissimilarity_match_oracle(dtype, include_t0):
         ora.append(np.array(o.frames)); gpu.append(fr)
     s0, s1 = 2, nfr - 2
     d = t.dissimilarity(s0, s1)
-    assert d.shape == (5, 5) and np.array_equal(d, d.T) and np.all(np.diag(d) == 0.0)
+    assert d.shape == (10, 10) and np.array_equal(d, d.T) and np.all(np.diag(d) == 0.0)
     for k in range(w.batch):
         for j in range(k + 1, w.batch):
             # the reduction alone (same frames in, different summation order): rounding level
@@ -880,7 +880,8 @@ def test_batched_potential_build_is_bit_identical_to_one_entry_at_a_time(idx, sh
 @pytest.mark.parametrize("tblock", [1, 2])
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("shape,bc,batch", [((72, 40, 37), BCS[0], 2), ((136, 70, 21), BCS[3], 1), ((64, 64, 16), BCS[1], 3),
-                                            ((128, 128, 40), BCS[2], 2), ((40, 24, 5), BCS[4], 1)])
+                                            ((128, 128, 40), BCS[2], 2), ((40, 24, 5), BCS[4], 1), ((132, 66, 9), BCS[2], 1),
+                                            ((64, 32, 12), BCS[2], 2), ((8, 8, 6), BCS[2], 1)])
 def test_iteration_barrier_variants_are_bit_identical(tblock, dtype, shape, bc, batch):
     """tdse_set_option("variant"): the fused kernel with the per-plane block barrier (2) and with the split arrive / wait
     mbarrier (1) do the same arithmetic in the same order -- every bit of psi and of the detector output must agree, over
@@ -907,7 +908,7 @@ def test_iteration_barrier_variants_are_bit_identical(tblock, dtype, shape, bc, 
     for v, res in zip(variants[1:], out[1:]):
         for b in range(batch):
             for x0, x1 in zip(out[0][b], res[b]):
-                assert np.array_equal(x0, x1), "variant %d, entry %d" % (v, b)
+                assert np.array_equal(x0, x1), "variant %s, entry %d" % (v, b)
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
