@@ -292,14 +292,19 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
     unsigned dpar = 0;                               // SPLIT: phase parity of iter_done
     int xw = 0, xr = PS;
 
-    unsigned out_pb = (unsigned)(Z0 - H - NS) * plane_bytes;   // byte offset of plane p-NS (wraps harmlessly while p-NS < Z0)
+    // Address of the thread's upper row in plane p-NS of R-out, advanced by one plane per iteration (while p-NS < Z0 it points
+    // below the chunk and is not dereferenced).  Everything a thread stores sits at a uniform or per-thread constant distance
+    // from it -- lower row, I-out one plane further, periodic images -- so a store costs one 64-bit add instead of an
+    // offset multiply-add chain (the stores and their address arithmetic are 16 % of the instruction stream).
+    char* out_r = oR + (long long)(Z0 - H - NS) * (long long)plane_bytes + goff[0];
+    const long long i_from_r = (oI - oR) + (long long)plane_bytes;   // I-out plane p-NS+1 relative to R-out plane p-NS
+    const unsigned row_bytes = goff[1] - goff[0];
 
     // the thread's two rows of a finished plane -> global memory, plus their periodic images inside the frame
-    auto store_rows = [&](char* base, unsigned pb, const V4 (&out)[2]) {
+    auto store_rows = [&](char* d0, const V4 (&out)[2]) {
         // predicated 16-byte stores, no divergent branches (a branch region per row and image cost more than the
         // stores themselves: profiles/README.md); only warps that hold a y-face row enter the y-image part
-        char* const d0 = base + (size_t)(pb + goff[0]);
-        char* const d1 = base + (size_t)(pb + goff[1]);
+        char* const d1 = d0 + row_bytes;
         st_global_pred(d0, out[0], core[0]);
         st_global_pred(d1, out[1], core[1]);
         if (warp_img_x) {
@@ -395,7 +400,7 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
             }
             if (!SPLIT && s == NS - 1) {             // I^{n+T-1/2} at plane p-NS+1
                 const int pz = p - (NS - 1);
-                if (pz >= Z0 && pz < Z0 + bzc) store_rows(oI, out_pb + plane_bytes, out);
+                if (pz >= Z0 && pz < Z0 + bzc) store_rows(out_r + i_from_r, out);
             }
             if (s == NS) {                           // R^{n+T} at plane p-NS
                 if (SPLIT) {
@@ -403,13 +408,13 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
                     __syncwarp();
                     if (lane == 0) mbar_arrive(iter_done);
                     const int pzi = p - (NS - 1);
-                    if (pzi >= Z0 && pzi < Z0 + bzc) store_rows(oI, out_pb + plane_bytes, nw.f[NS - 1]);
+                    if (pzi >= Z0 && pzi < Z0 + bzc) store_rows(out_r + i_from_r, nw.f[NS - 1]);
                 }
                 const int pz = p - NS;
-                if (pz >= Z0 && pz < Z0 + bzc) store_rows(oR, out_pb, out);
+                if (pz >= Z0 && pz < Z0 + bzc) store_rows(out_r, out);
             }
         }
-        out_pb += plane_bytes;
+        out_r += plane_bytes;
         ro_prev = ro_cur; ro_cur = ring_next(ro_cur); ro_fill = ring_next(ro_fill);
         if (++sl_cur == RD) { sl_cur = 0; par ^= 1u; }
         if (++sl_fill == RD) sl_fill = 0;
