@@ -530,8 +530,10 @@ def main():
                 "traffic": traffic, "kernel": kname, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes_per_launch, "avg_launch_ms": avg_launch_s * 1e3,
                 "dram_gbs": dram_bytes / avg_launch_s / 1e9, "dram_frac": dram_bytes / avg_launch_s / 1e9 / peak,
-                "dram_bytes_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum (profiles/roofline_traffic.csv)"
-                                     if traffic is not None else "compulsory bytes per launch on a flat layout (no ncu capture of this workload)",
+                "dram_bytes_source": ("ncu dram__bytes_read.sum + dram__bytes_write.sum (profiles/roofline_traffic.csv)"
+                                      if traffic is not None else "compulsory bytes per launch on a flat layout (no ncu capture of this workload)")
+                                     + ("" if 5 * w.cells * w.batch * wbytes > 4 * 126e6 else
+                                        "; ncu replays with cold caches, live this working set stays in L2: dram_gbs / dram_frac overstate what DRAM moves"),
                 "step_loop_gcell_per_s": step_value,
                 "frac_of_8TBps_nominal": achieved / 8000.0}
 

@@ -953,12 +953,13 @@ int tdse_set_potential_cell(tdse_ctx* c, int b, const double* cell, int on_devic
         cell_dev = c->cell_stage;
     }
     CellParams p{mx, my, mz, ax, ay, az, x0, y0, z0, vmin, vmax};
-    const unsigned nblk = (unsigned)((c->g.cells + 255) / 256);
+    const dim3 cgrid((unsigned)((c->g.nx + 31) / 32), (unsigned)((c->g.ny + 7) / 8), (unsigned)((c->g.nz + kCellSeg - 1) / kCellSeg));
+    if (cgrid.y > 65535 || cgrid.z > 65535) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: grid too large");
     void* dst = entry_ptr(c, c->V, b0);
     if (c->dtype == TDSE_F32)
-        potential_cell_kernel<float><<<nblk, 256, 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, cell_dev, p, static_cast<float*>(dst));
+        potential_cell_kernel<float><<<cgrid, dim3(32, 8), 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, cell_dev, p, static_cast<float*>(dst));
     else
-        potential_cell_kernel<double><<<nblk, 256, 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, cell_dev, p, static_cast<double*>(dst));
+        potential_cell_kernel<double><<<cgrid, dim3(32, 8), 0, c->stream>>>(c->g, c->m.dx, c->m.dy, c->m.dz, cell_dev, p, static_cast<double*>(dst));
     CU_LAUNCH_CHECK(c);
     for (int e = b0 + 1; e < b1; ++e)
         CU_TRY(c, cudaMemcpyAsync(entry_ptr(c, c->V, e), dst, (size_t)c->g.pcells * c->w, cudaMemcpyDeviceToDevice, c->stream));

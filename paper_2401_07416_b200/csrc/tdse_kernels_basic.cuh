@@ -13,9 +13,9 @@ struct AtomRec { double x, y, z, Z, soft2, screen; };   // same layout as tdse_a
 // Bound by the fp64 pipe, so the work per cell-atom pair is cut down to ~35 fp64 instructions without branches:
 //   * a thread owns CELLS consecutive cells along x and shares the y/z part of the distance among them;
 //   * atoms are staged through shared memory in chunks with 1/lambda precomputed;
-//   * inverse square roots: the hardware seed (MUFU.RSQ64H through rsqrt.approx.ftz.f64) + one third-order step;
-//   * exp(-r/lambda): x = n ln2/128 + r, exp(x) = 2^(n div 128) * T[n mod 128] * (1 + q(r)), T[j] = 2^(j/128) in shared
-//     memory, q = expm1 as a degree-5 polynomial on |r| <= ln2/256 (remainder < 6e-19);
+//   * r and 1/sqrt(r^2+s^2): the hardware seed (MUFU.RSQ64H through rsqrt.approx.ftz.f64) + one third-order step each;
+//   * exp(-r/lambda): x = n ln2/256 + r, exp(x) = 2^(n div 256) * T[n mod 256] * (1 + q(r)), T[j] = 2^(j/256) in shared
+//     memory, q = expm1 as a degree-4 polynomial on |r| <= ln2/512 (remainder < 4e-17);
 //   * nearest image by the round-to-nearest-even magic constant instead of rint.
 // Double accumulate in list order, one rounding to `real`.  One launch covers every batch entry (blockIdx.y); the
 // sum may start from a per-cell prefix (the atoms all entries share, summed once: prefix_out mode) -- the same sequence of
@@ -39,25 +39,35 @@ __device__ __forceinline__ double rsqrt_pos(double a)
     return fma(y * e, p, y);
 }
 
-// exp(x) for -30000 < x <= 0 with the 2^(j/128) table `T` (shared memory): x = n ln2/128 + r, |r| <= ln2/256, and
-// exp(x) = 2^(n div 128) * T[n mod 128] * (1 + q(r)), q = expm1 as a degree-5 polynomial (remainder r^6/720 < 6e-19).
-// r comes from one fma with ln2/128 rounded to double: its error, |n| * 2^-60, stays below 2e-15 for every term that
+// sqrt(a) for normal a > 0 from the same seed: a y is already sqrt(a) to 22 bits, and sqrt(a) = a y (1 + e/2 + 3 e^2/8)
+__device__ __forceinline__ double sqrt_pos(double a)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    const double t = a * y;
+    const double e = fma(-t, y, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    return fma(t * e, p, t);
+}
+
+// exp(x) for -30000 < x <= 0 with the 2^(j/256) table `T` (shared memory): x = n ln2/256 + r, |r| <= ln2/512, and
+// exp(x) = 2^(n div 256) * T[n mod 256] * (1 + q(r)), q = expm1 as a degree-4 polynomial (remainder r^5/120 < 4e-17).
+// r comes from one fma with ln2/256 rounded to double: its error, |n| * 2^-61, stays below 2e-15 for every term that
 // is not itself below 1e-16 (|x| < 37).  Below x = -708 the result stays near 2^-1022, which no sum registers.  exp(-0) = 1.
-constexpr int kExpTable = 128;
+constexpr int kExpTable = 256;
 
 __device__ __forceinline__ double exp_nonpositive(double x, const double* __restrict__ T)
 {
     double t = fma(x, (double)kExpTable * 1.4426950408889634074, kRoundMagic);
-    const int n = max(__double2loint(t), -1022 * kExpTable);        // n = 128 k + j; k >= -1022 keeps the result a normal number
+    const int n = max(__double2loint(t), -1022 * kExpTable);        // n = 256 k + j; k >= -1022 keeps the result a normal number
     t -= kRoundMagic;
     const double r = fma(t, -0.69314718055994530942 / (double)kExpTable, x);
-    double p = fma(r, 1.0 / 120.0, 1.0 / 24.0);
-    p = fma(p, r, 1.0 / 6.0);
+    double p = fma(r, 1.0 / 24.0, 1.0 / 6.0);
     p = fma(p, r, 0.5);
     p = fma(p, r, 1.0);
     const double s = T[n & (kExpTable - 1)];
-    const double v = fma(s, p * r, s);                              // 2^(j/128) e^r in [0.5, 2)
-    return __hiloint2double(__double2hiint(v) + ((n >> 7) << 20), __double2loint(v));   // * 2^k
+    const double v = fma(s, p * r, s);                              // 2^(j/256) e^r in [0.5, 2)
+    return __hiloint2double(__double2hiint(v) + ((n >> 8) << 20), __double2loint(v));   // * 2^k
 }
 
 // distance from coordinate a to the interval [lo, hi] along one axis (nearest periodic image if L > 0)
@@ -106,7 +116,7 @@ potential_build_kernel(Grid g, double dx, double dy, double dz, const AtomRec* _
     const double lox = (bx * kPotBX * CELLS - 1) * dx, hix = ((bx + 1) * kPotBX * CELLS) * dx;
     const double loy = (by * kPotBY - 1) * dy, hiy = ((by + 1) * kPotBY) * dy;
     const double loz = (bz * kPotBZ - 1) * dz, hiz = ((bz + 1) * kPotBZ) * dz;
-    static_assert(kExpTable == 128, "n >> 7 above");
+    static_assert(kExpTable == 256, "n >> 8 above");
     if (threadIdx.x < kExpTable) s_exp2[threadIdx.x] = exp2((double)threadIdx.x / (double)kExpTable);
     double sum[CELLS], xs[CELLS];
 #pragma unroll
@@ -163,7 +173,7 @@ potential_build_kernel(Grid g, double dx, double dy, double dz, const AtomRec* _
                 double ddx = xs[e] - A.x;
                 if (perx) ddx = fma(-Lx, fma(ddx, iLx, kRoundMagic) - kRoundMagic, ddx);
                 const double r2 = fma(ddx, ddx, yz2);
-                double r = r2 * rsqrt_pos(r2);
+                double r = sqrt_pos(r2);
                 if (HAS_CUT) {
                     // the cutoff is defined on r = sqrt(r2) (correctly rounded): decide on r2 unless it is a tie
                     if (fabs(r2 - rc2) <= 1e-12 * rc2) r = sqrt(r2);
@@ -203,42 +213,57 @@ __global__ void common_prefix_kernel(const AtomRec* __restrict__ atoms, const At
 // Potential from a unit-cell grid (PAPER.md:148, 213 step (ii): expansion and interpolation of the DFT potential
 // onto the mesh; reading 24): cell[mz][my][mx] doubles at spacings (ax/mx, ay/my, az/(mz-1)), periodic
 // in x and y, nearest plane beyond the cell in z, trilinear interpolation at (i dx - x0, j dy - y0, k dz - z0),
-// clamp, one rounding to `real`.  One thread per cell; the gather hits L2 (a unit cell is small).
+// clamp, one rounding to `real`.  The gather hits L1 / L2 (a unit cell is small).
 // ---------------------------------------------------------------------------------------------
 struct CellParams { int mx, my, mz; double ax, ay, az, x0, y0, z0, vmin, vmax; };
+
+// Block (32, 8): thread (tx, ty) owns the mesh column (i, j) and a z segment of `zs` planes (blockIdx.z): everything that
+// depends on x and y only -- the two periodic cell indices and weights per axis, the image offsets of the storage frame -- is
+// computed once per column, the march over k keeps the z part.
+constexpr int kCellSeg = 32;
 
 template <typename real>
 __global__ void __launch_bounds__(256)
 potential_cell_kernel(Grid g, double dx, double dy, double dz, const double* __restrict__ cell, CellParams p,
                       real* __restrict__ V /* entry base */)
 {
-    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= g.cells) return;
-    const long long t = c / g.nx;
-    const int i = (int)(c - t * g.nx);
-    const int k = (int)(t / g.ny), j = (int)(t - (long long)k * g.ny);
+    const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y;
+    if (i >= g.nx || j >= g.ny) return;
+    const int k0 = blockIdx.z * kCellSeg, k1 = min(k0 + kCellSeg, g.nz);
     const double hx = p.ax / p.mx, hy = p.ay / p.my, hz = (p.mz > 1) ? p.az / (p.mz - 1) : 1.0;
     const double u = (i * dx - p.x0) / hx, v = (j * dy - p.y0) / hy;
-    const double w = fmin(fmax((k * dz - p.z0) / hz, 0.0), (double)(p.mz - 1));
     const double fu = floor(u), fv = floor(v);
-    const double tu = u - fu, tv = v - fv;
-    int iw0 = min((int)floor(w), p.mz > 1 ? p.mz - 2 : 0);
-    const double tw = (p.mz > 1) ? w - (double)iw0 : 0.0;
-    const int iw1 = (p.mz > 1) ? iw0 + 1 : 0;
+    const double tu = u - fu, tv = v - fv, su = 1.0 - tu, sv = 1.0 - tv;
     // periodic cell index of floor(u): fu - mx * floor(fu / mx), exact in double for any mesh (no 64-bit integer division)
     const int iu0 = (int)(fu - (double)p.mx * floor(fu / (double)p.mx));
     const int iv0 = (int)(fv - (double)p.my * floor(fv / (double)p.my));
     const int iu1 = iu0 + 1 == p.mx ? 0 : iu0 + 1, iv1 = iv0 + 1 == p.my ? 0 : iv0 + 1;
-    auto at = [&](int a, int b, int cz) { return __ldg(cell + ((long long)cz * p.my + b) * p.mx + a); };
-    // same grouping as the definition: x, then y, then z; products and sums kept separate (no contraction)
-    const double c00 = __dadd_rn(__dmul_rn(at(iu0, iv0, iw0), 1.0 - tu), __dmul_rn(at(iu1, iv0, iw0), tu));
-    const double c10 = __dadd_rn(__dmul_rn(at(iu0, iv1, iw0), 1.0 - tu), __dmul_rn(at(iu1, iv1, iw0), tu));
-    const double c01 = __dadd_rn(__dmul_rn(at(iu0, iv0, iw1), 1.0 - tu), __dmul_rn(at(iu1, iv0, iw1), tu));
-    const double c11 = __dadd_rn(__dmul_rn(at(iu0, iv1, iw1), 1.0 - tu), __dmul_rn(at(iu1, iv1, iw1), tu));
-    const double c0 = __dadd_rn(__dmul_rn(c00, 1.0 - tv), __dmul_rn(c10, tv));
-    const double c1 = __dadd_rn(__dmul_rn(c01, 1.0 - tv), __dmul_rn(c11, tv));
-    const double val = __dadd_rn(__dmul_rn(c0, 1.0 - tw), __dmul_rn(c1, tw));
-    store_with_images(V, g, i, j, k, (real)fmin(fmax(val, p.vmin), p.vmax));
+    const int o00 = iv0 * p.mx + iu0, o01 = iv0 * p.mx + iu1, o10 = iv1 * p.mx + iu0, o11 = iv1 * p.mx + iu1;
+    const long long cplane = (long long)p.my * p.mx;
+    int ix = 0, jy = 0;                  // shifts of the periodic images this column also stores (0: none)
+    if (g.bcx == BC_PERIODIC) { if (i < PADX) ix = g.nx; else if (i >= g.nx - PADX) ix = -g.nx; }
+    if (g.bcy == BC_PERIODIC) { if (j < PADY) jy = g.ny * g.px; else if (j >= g.ny - PADY) jy = -g.ny * g.px; }
+    long long o = cell_offset(g, i, j, k0);
+    for (int k = k0; k < k1; ++k, o += g.pplane) {
+        const double w = fmin(fmax((k * dz - p.z0) / hz, 0.0), (double)(p.mz - 1));
+        const int iw0 = min((int)floor(w), p.mz > 1 ? p.mz - 2 : 0);
+        const double tw = (p.mz > 1) ? w - (double)iw0 : 0.0;
+        const double* __restrict__ c0p = cell + (long long)iw0 * cplane;
+        const double* __restrict__ c1p = (p.mz > 1) ? c0p + cplane : cell;
+        // same grouping as the definition: x, then y, then z; products and sums kept separate (no contraction)
+        const double c00 = __dadd_rn(__dmul_rn(__ldg(c0p + o00), su), __dmul_rn(__ldg(c0p + o01), tu));
+        const double c10 = __dadd_rn(__dmul_rn(__ldg(c0p + o10), su), __dmul_rn(__ldg(c0p + o11), tu));
+        const double c01 = __dadd_rn(__dmul_rn(__ldg(c1p + o00), su), __dmul_rn(__ldg(c1p + o01), tu));
+        const double c11 = __dadd_rn(__dmul_rn(__ldg(c1p + o10), su), __dmul_rn(__ldg(c1p + o11), tu));
+        const double c0 = __dadd_rn(__dmul_rn(c00, sv), __dmul_rn(c10, tv));
+        const double c1 = __dadd_rn(__dmul_rn(c01, sv), __dmul_rn(c11, tv));
+        const double val = __dadd_rn(__dmul_rn(c0, 1.0 - tw), __dmul_rn(c1, tw));
+        const real out = (real)fmin(fmax(val, p.vmin), p.vmax);
+        V[o] = out;
+        if (ix) V[o + ix] = out;
+        if (jy) V[o + jy] = out;
+        if (ix && jy) V[o + ix + jy] = out;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
