@@ -953,3 +953,45 @@ def test_streamed_frames_equal_the_flat_frame_mode_bit_for_bit(dtype, include_t0
         assert np.array_equal(again[b], want[b][:cap])
     t.set_frame_stream(0, 0)                               # off
     t.close()
+
+
+def test_batch_build_and_frame_stream_argument_errors_and_empty_lists():
+    """Host-side checks of the two round-2 calls: bad offsets / NULL / too few ring slots fail with TDSE_EINVAL and leave the
+    context usable; entries with an empty atom list get V = clamp(0) (or just the shared prefix when every list is short)."""
+    import ctypes as C
+    from paper_2401_07416_b200 import Tdse, TdseError, TDSE_EINVAL
+    w = make_config(3, n=(32, 32, 24), batch=3, dtype="f64")
+    t = make_ctx(w.nx, w.ny, w.nz, 3, w.dx, w.dt, "f64")
+    t.set_boundary(*w.bc, 2, 2, 0.05, 2)
+    atoms = np.ascontiguousarray(np.concatenate(w.atoms[:2]))
+    n0, n1 = w.atoms[0].shape[0], w.atoms[1].shape[0]
+    for bad in ([0, n0, n0 - 1, n0 + n1], [-1, n0, n0, n0 + n1]):
+        with pytest.raises(TdseError) as e:
+            t.set_potential_batch(atoms, bad, w.vmin, w.vmax)
+        assert e.value.code == TDSE_EINVAL
+    with pytest.raises(TdseError) as e:
+        t.set_potential_batch(atoms, [0, n0, n0, n0 + n1], 1.0, -1.0)      # vmin > vmax
+    assert e.value.code == TDSE_EINVAL
+    # entry 1 has no atoms at all
+    t.set_potential_batch(atoms, [0, n0, n0, n0 + n1], w.vmin, w.vmax)
+    assert np.array_equal(t.read_potential(1), np.zeros((w.nz, w.ny, w.nx)))
+    for b, lst in ((0, w.atoms[0]), (2, w.atoms[1])):
+        o = OracleRun(w.nx, w.ny, w.nz, w.dx, w.dt, bc=w.bc).set_potential_atoms(lst, w.vmin, w.vmax)
+        assert np.max(np.abs(t.read_potential(b) - o.V64)) <= 1e-13 * max(1.0, np.max(np.abs(o.V64)))
+    # frame stream: needs a buffer and >= 2 slots
+    buf = np.zeros((3, 4, w.ny, w.nx))
+    dp = C.POINTER(C.c_double)
+    assert t.L.tdse_set_frame_stream(t._h, buf.ctypes.data_as(dp), 4, 1, 1) == TDSE_EINVAL
+    assert t.L.tdse_set_frame_stream(t._h, None, 4, 2, 1) == TDSE_EINVAL
+    assert t.L.tdse_set_frame_stream(t._h, buf.ctypes.data_as(dp), -1, 2, 1) == TDSE_EINVAL
+    # still usable: pageable host buffer given directly through the C ABI, 2 slots for 4 frames
+    p = w.packet
+    t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], 0.0)
+    t.set_detector(3, 2, 8)
+    assert t.L.tdse_set_frame_stream(t._h, buf.ctypes.data_as(dp), 4, 2, 1) == 0
+    t.step(6)
+    n = C.c_int(0)
+    assert t.L.tdse_frames_sync(t._h, C.byref(n)) == 0 and n.value == 4
+    assert np.all(buf.sum(axis=(2, 3)) > 0)
+    assert t.L.tdse_set_frame_stream(t._h, None, 0, 0, 1) == 0      # off again before the buffer goes
+    t.close()
