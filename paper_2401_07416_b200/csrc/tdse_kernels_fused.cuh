@@ -300,24 +300,20 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
     const long long i_from_r = (oI - oR) + (long long)plane_bytes;   // I-out plane p-NS+1 relative to R-out plane p-NS
     const unsigned row_bytes = goff[1] - goff[0];
 
-    // the thread's two rows of a finished plane -> global memory, plus their periodic images inside the frame
-    auto store_rows = [&](char* d0, const V4 (&out)[2]) {
+    // one of the thread's two rows (j) of a finished plane -> global memory, plus its periodic images inside the frame;
+    // d0 = address of the thread's upper row in that plane
+    auto store_row = [&](char* d0, const V4& v, const int j) {
         // predicated 16-byte stores, no divergent branches (a branch region per row and image cost more than the
         // stores themselves: profiles/README.md); only warps that hold a y-face row enter the y-image part
-        char* const d1 = d0 + row_bytes;
-        st_global_pred(d0, out[0], core[0]);
-        st_global_pred(d1, out[1], core[1]);
-        if (warp_img_x) {
-            st_global_pred(d0 + img_x, out[0], core[0] && img_x);
-            st_global_pred(d1 + img_x, out[1], core[1] && img_x);
-        }
+        char* const d = j ? d0 + row_bytes : d0;
+        st_global_pred(d, v, core[j]);
+        if (warp_img_x) st_global_pred(d + img_x, v, core[j] && img_x);
         if (warp_img_y) {
-            st_global_pred(d0 + img_y[0], out[0], img_y[0]);
-            st_global_pred(d1 + img_y[1], out[1], img_y[1]);
-            st_global_pred(d0 + img_y[0] + img_x, out[0], img_y[0] && img_x);
-            st_global_pred(d1 + img_y[1] + img_x, out[1], img_y[1] && img_x);
+            st_global_pred(d + img_y[j], v, img_y[j]);
+            st_global_pred(d + img_y[j] + img_x, v, img_y[j] && img_x);
         }
     };
+    auto store_rows = [&](char* d0, const V4 (&out)[2]) { store_row(d0, out[0], 0); store_row(d0, out[1], 1); };
 
     // One iteration of the march: plane p = Z0-H+t has arrived.  `old`/`mid` hold planes p-s-2 / p-s-1 of
     // every stage s; `nw` receives plane p-s.  (old, mid, nw) rotate by renaming: see the calls below.
@@ -398,9 +394,18 @@ fdtd_fused_kernel(const FusedParams P, const __grid_constant__ CUtensorMap tmR,
                     if (!(SPLIT && s == 1)) *reinterpret_cast<V4*>(exch + (s - 1) * XD * PS + xw + soff + j * HP) = out[j];
                 }
             }
-            if (!SPLIT && s == NS - 1) {             // I^{n+T-1/2} at plane p-NS+1
-                const int pz = p - (NS - 1);
-                if (pz >= Z0 && pz < Z0 + bzc) store_rows(out_r + i_from_r, out);
+            // I^{n+T-1/2} of the PREVIOUS iteration (plane p-NS, the same plane index as this iteration's R-out) sits in the
+            // queue anyway: its two rows are stored here, spread over the stages, instead of right behind stage NS-1, so that
+            // the global stores of an iteration do not all leave in one burst at its end (measured: +3 to +7 % on the f32
+            // grids, profiles/r02_experiments.md).  The last iteration produces no valid I plane: nothing is left over.
+            constexpr int I0_AT = NS == 2 ? 1 : (sizeof(real) == 4 ? 2 : 1), I1_AT = NS == 2 ? 2 : 3;
+            if (!SPLIT && (s == I0_AT || s == I1_AT)) {
+                const int pz = p - NS;
+                if (pz >= Z0 && pz < Z0 + bzc) {
+                    char* const d = out_r + (i_from_r - (long long)plane_bytes);
+                    if (s == I0_AT) store_row(d, mid.f[NS - 1][0], 0);
+                    if (s == I1_AT) store_row(d, mid.f[NS - 1][1], 1);
+                }
             }
             if (s == NS) {                           // R^{n+T} at plane p-NS
                 if (SPLIT) {
