@@ -995,3 +995,40 @@ def test_batch_build_and_frame_stream_argument_errors_and_empty_lists():
     assert np.all(buf.sum(axis=(2, 3)) > 0)
     assert t.L.tdse_set_frame_stream(t._h, None, 0, 0, 1) == 0      # off again before the buffer goes
     t.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("shape,bc,batch", [((72, 40, 37), BCS[0], 2), ((136, 70, 21), BCS[2], 1), ((64, 32, 9), BCS[1], 3),
+                                            ((128, 128, 24), BCS[2], 1), ((8, 8, 5), BCS[3], 2)])
+def test_nothing_is_written_outside_the_workspace(shape, bc, batch, dtype):
+    """Guard bands on both sides of a caller-owned workspace (and between its five arrays there is none to spare: they are
+    contiguous) stay untouched through potential build, packet init, fused steps of both temporal blocks and the two-pass
+    kernel: the kernels advance store addresses from below the first plane of a chunk and must never dereference them there."""
+    import ctypes as C
+    import torch
+    from paper_2401_07416_b200 import binding as B
+    nx, ny, nz = shape
+    L = B.load()
+    code = B.TDSE_F32 if dtype == "f32" else B.TDSE_F64
+    nbytes = L.tdse_workspace_bytes(nx, ny, nz, batch, code, 1)
+    guard = 1 << 20
+    buf = torch.full((nbytes + 2 * guard,), 0xA5, dtype=torch.uint8, device="cuda")
+    assert (buf.data_ptr() + guard) % 256 == 0
+    h = C.c_void_p()
+    assert L.tdse_create(C.byref(h), nx, ny, nz, batch, 0.25, 0.004, 1.0, 1.0, code) == 0
+    assert L.tdse_bind(h, buf.data_ptr() + guard, nbytes, None) == 0
+    assert L.tdse_set_boundary(h, *bc, 2, 2, 0.07, 2) == 0
+    atoms = B.atoms_array(np.array([[nx * 0.1, ny * 0.1, nz * 0.1, 3.0, 0.2, 0.6], [0.3, 0.2, 0.1, 2.0, 0.1, 0.0]]))
+    assert L.tdse_set_potential(h, -1, atoms[0], atoms[1], -50.0, 0.0, 0.0) == 0
+    assert L.tdse_set_wavepacket(h, -1, nx * 0.12, ny * 0.12, nz * 0.1, 1.0, 0.0, 0.0, 1.0, 0.0) == 0
+    assert L.tdse_set_detector(h, 1, 3, 8) == 0
+    for kernel, tblock in ((2, 2), (2, 1), (1, 1)):
+        if kernel == 2 and not fused_eligible(nx, ny, dtype):
+            continue
+        assert L.tdse_set_option(h, b"kernel", kernel) == 0 and L.tdse_set_option(h, b"tblock", tblock) == 0
+        for variant in (1, 2):
+            assert L.tdse_set_option(h, b"variant", variant) == 0
+            assert L.tdse_step(h, 7) == 0
+    torch.cuda.synchronize()
+    assert bool((buf[:guard] == 0xA5).all()) and bool((buf[guard + nbytes:] == 0xA5).all())
+    L.tdse_destroy(h)
