@@ -226,6 +226,34 @@ def test_absorber_inside_the_step_vs_dense_linear_map(shape, bc, w_lo, w_hi, str
         assert rel_l2((alt @ np.concatenate([R0.ravel(), I0.ravel()]))[:N], want[:N]) > 1e-3
 
 
+@pytest.mark.parametrize("shape,bc,w_lo,w_hi,strength,power", ABSORBER_CASES)
+def test_norms_with_absorber_vs_dense_linear_map(shape, bc, w_lo, w_hi, strength, power):
+    """oracle_norm's look-ahead carries the mask (readings 6-7): I^{n+1/2} is what the next
+    eq (9) half-step WOULD store, D_M (I - A R), so
+        q_visscher = dV ( R.R + (D_M (I - A R)).I ),     q_paper = dV ( R.R + I.I ).
+    Built densely from dense_A and mask_table (neither is the oracle's code) on a state that has been stepped into the
+    absorber.  Dropping M from the look-ahead, or using it squared, each miss by > 1e-4 on these inputs."""
+    nx, ny, nz = shape
+    dx, dt = 0.3, 0.01
+    V = random_potential(41, (nz, ny, nx), -3.0, 1.0)
+    R0, I0 = random_state(42, (nz, ny, nx))
+    o = OracleRun(nx, ny, nz, dx, dt, bc=bc, absorb_lo=w_lo, absorb_hi=w_hi, strength=strength, power=power)
+    o.set_potential_grid(V).set_state(R0, I0).step(5)
+    c, _, _, cv = oracle.coefficients(dx, dt, 1.0, 1.0)
+    A = dense_A(nx, ny, nz, bc, c, cv, V)
+    m = np.repeat(mask_table(nz, w_lo, w_hi, strength, power), ny * nx)
+    R, I = np.asarray(o.R, dtype=np.float64).ravel(), np.asarray(o.I, dtype=np.float64).ravel()
+    look = I - A @ R
+    dV = dx ** 3
+    want_v = dV * (R @ R + (m * look) @ I)
+    want_p = dV * (R @ R + I @ I)
+    qv, qp = o.norm()
+    assert abs(qv - want_v) <= 1e-13 * abs(want_v)
+    assert abs(qp - want_p) <= 1e-13 * abs(want_p)
+    for alt in (dV * (R @ R + look @ I), dV * (R @ R + (m * m * look) @ I)):     # no mask / mask twice
+        assert abs(alt - want_v) > 1e-4 * abs(want_v)
+
+
 def test_stationary_eigenvector_has_constant_visscher_density():
     nx, ny, nz = 4, 3, 5
     bc = (DIRICHLET, PERIODIC, DIRICHLET)
