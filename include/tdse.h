@@ -219,6 +219,44 @@ int tdse_frames_sync(tdse_ctx* ctx, int* nframes);
  * Synchronises.  Errors: TDSE_ESTATE (frame mode off), TDSE_EINVAL (window exceeds the frames kept). */
 int tdse_dissimilarity(tdse_ctx* ctx, int first_frame, int last_frame, double* d_host);
 
+/* Eq (16) for callers that must not allocate GPU memory.
+ *
+ * Who this is for.  tdse_dissimilarity() sizes a per-context reduction buffer with cudaMalloc the first time it sees a
+ * new batch x window.  Some programs cannot let a library do that: a job that has handed (nearly) all of the 180 GB to
+ * the grids, as the fill-HBM configuration does, has nothing left for cudaMalloc to find; a host whose device memory
+ * is owned by one pool (an inference server, a torch caching allocator with a hard cap) treats a side allocation as a
+ * budget violation or an out-of-memory risk; and cudaMalloc/cudaFree stall the whole device, which a loop that is
+ * stepping other contexts on other streams cannot afford.  This call does the same computation with the same kernels
+ * and never calls cudaMalloc, cudaFree or any other allocating routine.
+ *
+ * How.  The per-(pair, frame) partial results go to a fixed array of TDSE_STATIC_SCRATCH_DOUBLES doubles (2 MiB) that
+ * is part of the library image: every GPU that loads libtdse holds those 2 MiB from load until the process exits,
+ * whether or not this call is ever made.  Inputs and outputs stay the caller's:
+ *   frames_device  DEVICE, [batch][frames_per_entry][ny][nx] doubles (the layout tdse_frames_device returns), read only
+ *   d_device       DEVICE, batch*batch doubles, written: symmetric, zero diagonal, same values as tdse_dissimilarity
+ *   dA             area of one detector pixel (dx*dy)
+ *   cuda_stream    a cudaStream_t passed as void* (NULL = legacy default stream); the work is enqueued there and the
+ *                  call returns without synchronising -- d_device is ready when that stream reaches this point.
+ * Both pointers must belong to the device that is current in the calling thread.
+ *
+ * Limit: batch*batch*(last_frame-first_frame+1) <= TDSE_STATIC_SCRATCH_DOUBLES (e.g. 32 trajectories x the paper's 250
+ * frames); anything larger is refused with TDSE_EINVAL and a message, nothing is launched.
+ *
+ * Sharing.  There is one array per GPU and every call on that GPU uses it.  A call overwrites each element it later
+ * reads, so nothing has to be cleared and what the previous call left behind is never seen.  Two calls that can be in
+ * flight on the same GPU at once (different streams, or two host threads) race on the array and both results are
+ * garbage: put them on one stream, or order them with events.
+ *
+ * First call.  The first call on each GPU looks up the array's device address (cudaGetSymbolAddress, which may also
+ * make the CUDA runtime load the module); later calls reuse it.  Make that first call during set-up, before starting
+ * any stream capture on that GPU.
+ *
+ * Errors: TDSE_EINVAL (NULL, sizes < 1, bad window, over the limit, pointer not device memory of the current
+ * device), TDSE_ECUDA.  Text goes to the global slot: tdse_last_error(NULL). */
+enum { TDSE_STATIC_SCRATCH_DOUBLES = 262144 };
+int tdse_dissimilarity_static(const double* frames_device, int batch, int frames_per_entry, int ny, int nx, double dA,
+                              int first_frame, int last_frame, double* d_device, void* cuda_stream);
+
 /* Device pointers to the detector image [batch][ny][nx] and trace [batch][max_samples] (doubles);
  * valid until the next tdse_set_detector or tdse_destroy.  Does not synchronise. */
 int tdse_detector_device(tdse_ctx* ctx, double** image_device, double** trace_device, int* max_samples);

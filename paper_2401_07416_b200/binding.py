@@ -31,7 +31,10 @@ SYMBOLS = [
     "tdse_detector_read", "tdse_detector_device", "tdse_read_psi", "tdse_read_potential",
     "tdse_norm", "tdse_set_option", "tdse_get_info", "tdse_last_error",
     "tdse_set_frames", "tdse_frames_read", "tdse_frames_device", "tdse_dissimilarity", "tdse_set_spacing", "tdse_set_potential_cell", "tdse_set_potential_batch", "tdse_set_frame_stream", "tdse_frames_sync",
+    "tdse_dissimilarity_static",
 ]
+
+TDSE_STATIC_SCRATCH_DOUBLES = 262144   # include/tdse.h: size of the fixed scratch array behind tdse_dissimilarity_static
 
 
 class TdseError(RuntimeError):
@@ -81,6 +84,7 @@ def load():
     L.tdse_set_frame_stream.argtypes = [vp, dp, C.c_int, C.c_int, C.c_int]
     L.tdse_frames_sync.argtypes = [vp, ip]
     L.tdse_dissimilarity.argtypes = [vp, C.c_int, C.c_int, dp]
+    L.tdse_dissimilarity_static.argtypes = [vp] + [C.c_int] * 4 + [C.c_double, C.c_int, C.c_int, vp, vp]
     L.tdse_read_psi.argtypes = [vp, C.c_int, vp, vp]
     L.tdse_read_potential.argtypes = [vp, C.c_int, vp]
     L.tdse_norm.argtypes = [vp, C.c_int, dp, dp]
@@ -94,6 +98,26 @@ def load():
             f.restype = C.c_int
     _lib = L
     return L
+
+
+def dissimilarity_static(frames, first_frame, last_frame, dA, out, stream=None):
+    """tdse_dissimilarity_static: eq (16) for callers that may not allocate GPU memory (a job that gave all of HBM to the
+    grids, a process whose device memory belongs to one pool, a loop that cannot take cudaMalloc's device-wide stall).
+
+    frames: device tensor [batch][frames_per_entry][ny][nx], float64, contiguous; out: device tensor [batch][batch],
+    float64, contiguous -- both on the current device, both the caller's.  Nothing is allocated here or in the library:
+    the partial sums go to a fixed 2 MiB array inside libtdse.so that all calls on a GPU share (so calls that may
+    overlap on the GPU must be ordered by the caller).  Asynchronous on `stream`; raises TdseError(TDSE_EINVAL) when
+    batch*batch*frames exceeds TDSE_STATIC_SCRATCH_DOUBLES.  The first call on a GPU looks up the array's address and
+    belongs in set-up code, ahead of any stream capture."""
+    L = load()
+    batch, per_entry, ny, nx = (int(v) for v in frames.shape)
+    sptr = stream.cuda_stream if stream is not None else 0
+    code = L.tdse_dissimilarity_static(frames.data_ptr(), batch, per_entry, ny, nx, float(dA), int(first_frame),
+                                       int(last_frame), out.data_ptr(), sptr)
+    if code != TDSE_OK:
+        raise TdseError(code, "tdse_dissimilarity_static", (L.tdse_last_error(None) or b"").decode())
+    return out
 
 
 def atoms_array(atoms) -> "C.Array":

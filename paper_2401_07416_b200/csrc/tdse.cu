@@ -1370,3 +1370,96 @@ int tdse_get_info(const tdse_ctx* c, const char* key, long long* value)
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// tdse_dissimilarity_static: eq (16) without any allocation (include/tdse.h says who needs that and why).
+// The scratch that tdse_dissimilarity takes from cudaMalloc is this fixed array instead.  It lives in the module
+// image, so each GPU that loads the library carries it (2 MiB) until the process ends, and all calls on a GPU share it.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_static_scratch[TDSE_STATIC_SCRATCH_DOUBLES];
+
+namespace {
+
+// Device address of g_static_scratch on each GPU, filled in by the first call made with that GPU current.  In host
+// code `g_static_scratch` is only a handle for the runtime's symbol table -- handing it to a kernel as if it were a
+// pointer would make the kernel dereference a host address -- so the real address is asked for once per device
+// (the array has a different address in every device's copy of the module) and kept here.
+double* g_static_scratch_addr[kMaxDevices] = {};
+
+int static_scratch_for_current_device(double** out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(nullptr, TDSE_ECUDA, std::string("tdse_dissimilarity_static: cudaGetDevice: ") + cudaGetErrorString(e)
+                                         + " (no CPU fallback)");
+    }
+    if (dev < 0 || dev >= kMaxDevices) return fail(nullptr, TDSE_EINVAL, "tdse_dissimilarity_static: device ordinal out of range");
+    double* p = g_static_scratch_addr[dev];       // racing first calls would both store the same address
+    if (!p) {
+        e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_static_scratch);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return fail(nullptr, TDSE_ECUDA, std::string("tdse_dissimilarity_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+        }
+        g_static_scratch_addr[dev] = p;
+    }
+    *out = p;
+    return TDSE_OK;
+}
+
+// true if p is device (or managed) memory that the current device `dev` owns
+bool is_memory_of_device(const void* p, int dev)
+{
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    if (a.type == cudaMemoryTypeManaged) return true;
+    return a.type == cudaMemoryTypeDevice && a.device == dev;
+}
+
+}  // namespace
+
+extern "C" int tdse_dissimilarity_static(const double* frames_device, int batch, int frames_per_entry, int ny, int nx,
+                                         double dA, int first_frame, int last_frame, double* d_device, void* cuda_stream)
+{
+    const char* who = "tdse_dissimilarity_static: ";
+    if (!frames_device || !d_device) return fail(nullptr, TDSE_EINVAL, std::string(who) + "NULL");
+    if (batch < 1 || frames_per_entry < 1 || ny < 1 || nx < 1 || !(dA > 0.0))
+        return fail(nullptr, TDSE_EINVAL, std::string(who) + "batch, frames_per_entry, ny, nx must be >= 1 and dA > 0");
+    if ((long long)ny * nx > std::numeric_limits<int>::max())
+        return fail(nullptr, TDSE_EINVAL, std::string(who) + "ny*nx exceeds 2^31 - 1");
+    if (first_frame < 0 || last_frame < first_frame || last_frame >= frames_per_entry)
+        return fail(nullptr, TDSE_EINVAL, std::string(who) + "frame window outside [0, frames_per_entry)");
+    const int nwin = last_frame - first_frame + 1;
+    const long long need = (long long)batch * batch * nwin;
+    if (nwin > 65535) return fail(nullptr, TDSE_EINVAL, std::string(who) + "more than 65535 frames in the window");
+    if (need > (long long)TDSE_STATIC_SCRATCH_DOUBLES) {
+        char msg[256];
+        snprintf(msg, sizeof msg, "%sbatch*batch*frames = %lld exceeds the fixed scratch of %d doubles; shorten the window, "
+                 "split the batch, or use tdse_dissimilarity (which allocates)", who, need, (int)TDSE_STATIC_SCRATCH_DOUBLES);
+        return fail(nullptr, TDSE_EINVAL, msg);
+    }
+    double* inner = nullptr;
+    const int rc = static_scratch_for_current_device(&inner);     // first call on this GPU: looks the address up
+    if (rc) return rc;
+    int dev = -1;
+    cudaGetDevice(&dev);
+    if (!is_memory_of_device(frames_device, dev) || !is_memory_of_device(d_device, dev))
+        return fail(nullptr, TDSE_EINVAL, std::string(who) + "frames_device and d_device must be device memory of the current device");
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const int npix = ny * nx;
+    const int tiles = (batch + kDisTile - 1) / kDisTile;
+    // Same two kernels, launch shapes and summation order as tdse_dissimilarity.  The first writes every
+    // inner[(k*batch + j)*nwin + s] with j >= k, the second reads exactly those: no element of the shared array is read
+    // before this call has written it, whatever an earlier call left there.
+    dissimilarity_inner_kernel<<<dim3((unsigned)(tiles * tiles), (unsigned)nwin), 256, 0, stream>>>(
+        frames_device, batch, (long long)frames_per_entry * npix, npix, dA, first_frame, nwin, inner);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) {
+        dissimilarity_finish_kernel<<<(batch * batch + 127) / 128, 128, 0, stream>>>(inner, batch, nwin, d_device);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) return fail(nullptr, TDSE_ECUDA, std::string(who) + "kernel launch: " + cudaGetErrorString(e));
+    return TDSE_OK;
+}
