@@ -23,7 +23,9 @@
  *     tdse_bind() stays owned by the caller and must outlive the context.
  *   - All work is enqueued on the stream given to tdse_bind() (default: the legacy null stream).
  *     tdse_step() is asynchronous; calls that return data to the host synchronise that stream.
- *   - One context is not thread-safe; distinct contexts are independent.
+ *   - One context is not thread-safe; distinct contexts are independent and may be driven from different host
+ *     threads.  The context-free error slot (tdse_last_error(NULL): tdse_create failures, tdse_dissimilarity_static)
+ *     is per host thread.  tdse_dissimilarity_static shares one scratch array per GPU across all callers (see there).
  *   - There is no CPU fallback: every call needs a CUDA device and fails with TDSE_ECUDA without one.
  */
 #ifndef TDSE_H
@@ -157,7 +159,9 @@ int tdse_set_wavepacket(tdse_ctx* ctx, int b, double x0, double y0, double z0, d
                         double kx, double ky, double kz, double amplitude);
 
 /* Raw state for entry b (b = -1: the same state for all entries): R^n and I^{n-1/2}, nx*ny*nz values
- * each of the context dtype, [z][y][x].  Resets the step counter and the detector. */
+ * each of the context dtype, [z][y][x].  Resets the step counter and the detector: this is a fresh start from a given
+ * wavefunction, not a checkpoint restore -- the sampling phase, the accumulated image, the trace and the frames begin
+ * again at zero, so a caller that resumes a run keeps its own copy of those and adds to it. */
 int tdse_set_state(tdse_ctx* ctx, int b, const void* R, const void* I_half, int on_device);
 
 /* Detector plane k_plane (0 <= k_plane < nz), sampled after every `every`-th full step counted from the
@@ -205,7 +209,9 @@ int tdse_frames_device(tdse_ctx* ctx, double** frames_device, int* max_frames, i
  * waits only when it comes back to a slot whose copy has not left yet.  Frames beyond `capacity` are dropped.  The buffer
  * belongs to the caller and must stay valid until tdse_frames_sync has returned after the last step (or the mode is
  * switched off with capacity = 0).  Excludes tdse_set_frames / tdse_dissimilarity (which need the frames on the device).
- * Resets the detector.  Errors: TDSE_EINVAL, TDSE_ENOMEM, TDSE_ECUDA. */
+ * Resets the detector.  When capacity * ny * nx * 8 bytes exceeds the device's 2-D copy pitch limit (cudaDevAttrMaxPitch,
+ * 2^31 - 1 bytes) a slot leaves as one copy per entry instead of one strided copy; the result is the same.
+ * Errors: TDSE_EINVAL, TDSE_ENOMEM, TDSE_ECUDA. */
 int tdse_set_frame_stream(tdse_ctx* ctx, double* frames_host, int capacity, int ring_slots, int include_t0);
 
 /* Wait until every frame sampled so far has landed in the host buffer of tdse_set_frame_stream; *nframes = frames kept per
@@ -286,7 +292,8 @@ int tdse_set_option(tdse_ctx* ctx, const char* key, long long value);
 
 /* Introspection: "launches" (kernels launched by this context so far), "steps" (full steps since the last
  * reset), "kernel" / "tblock" (what tdse_step used last), "pingpong" (1 if 5-array workspace),
- * "tile_x", "tile_y", "z_chunks" (fused launch shape used last).  Errors: TDSE_EINVAL. */
+ * "tile_x", "tile_y", "z_chunks" (fused launch shape used last), "nsamples" (detector samples taken since the last
+ * reset), "nframes" (frames taken since the last reset, kept or not).  Errors: TDSE_EINVAL. */
 int tdse_get_info(const tdse_ctx* ctx, const char* key, long long* value);
 
 /* Text of the last error on this context ("" if none).  Never NULL.  ctx may be NULL (global slot used

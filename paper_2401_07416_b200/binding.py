@@ -270,13 +270,17 @@ class Tdse:
     def set_frame_stream(self, capacity, ring_slots=4, include_t0=True, pinned=True):
         """Streamed frame mode: torch owns the (page-locked) host buffer [batch][capacity][ny][nx]; the library fills it."""
         torch = self._torch
-        self._frames_host = None
+        fresh = None
         if capacity > 0:
             buf = torch.empty((self.batch, int(capacity), self.ny, self.nx), dtype=torch.float64)
-            self._frames_host = buf.pin_memory() if pinned else buf
-        ptr = C.cast(self._frames_host.data_ptr(), C.POINTER(C.c_double)) if capacity > 0 else None
+            fresh = buf.pin_memory() if pinned else buf
+        ptr = C.cast(fresh.data_ptr(), C.POINTER(C.c_double)) if capacity > 0 else None
+        # The previous host buffer stays referenced until the library call has returned: that call is what waits for
+        # copies still in flight into it (tdse.h: the buffer must stay valid until then), and torch's pinned-memory
+        # allocator, which knows nothing of the library's copy stream, could otherwise hand the block out again.
         self._check(self.L.tdse_set_frame_stream(self._h, ptr, int(capacity), int(ring_slots), 1 if include_t0 else 0),
                     "tdse_set_frame_stream")
+        self._frames_host = fresh
 
     def frames_sync(self) -> np.ndarray:
         """Frames landed so far as a numpy view [batch][nframes][ny][nx] of the host buffer."""

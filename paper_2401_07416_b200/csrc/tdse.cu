@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -23,7 +24,7 @@ using namespace tdse;
 
 namespace {
 
-std::string g_create_error;
+thread_local std::string g_create_error;    // the context-free error slot (tdse_last_error(NULL)): one per host thread
 
 constexpr size_t kAlign = 256;
 constexpr int kMaxDevices = 64;
@@ -81,6 +82,7 @@ struct tdse_ctx {
     double* fs_ring = nullptr;
     double* fs_host = nullptr;
     int fs_slots = 0, fs_capacity = 0;
+    bool fs_copy2d = true;              // one strided 2-D copy per slot (host pitch within cudaDevAttrMaxPitch), else one copy per entry
     cudaStream_t fs_stream = nullptr;
     std::vector<cudaEvent_t> fs_written, fs_copied;
     std::vector<char> fs_busy;          // fs_copied[slot] has been recorded since the last reset
@@ -100,16 +102,23 @@ struct tdse_ctx {
 namespace {
 
 // Every entry point runs on the context's device whatever device the caller has current, and restores the caller's.
+// If the switch cannot be made the entry point must not run at all (it would launch on some other device against this
+// device's pointers): ok() is false and ENTER_DEVICE returns TDSE_ECUDA.
 struct DeviceScope {
     int prev = -1;
     bool switched = false;
+    cudaError_t err = cudaSuccess;
     explicit DeviceScope(const tdse_ctx* c)
     {
         if (!c) return;
-        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; return; }
-        if (prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+        if ((err = cudaGetDevice(&prev)) != cudaSuccess) { cudaGetLastError(); prev = -1; return; }
+        if (prev != c->device) {
+            if ((err = cudaSetDevice(c->device)) != cudaSuccess) { cudaGetLastError(); return; }
+            switched = true;
+        }
     }
-    ~DeviceScope() { if (switched) cudaSetDevice(prev); }
+    bool ok() const { return err == cudaSuccess; }
+    ~DeviceScope() { if (switched && cudaSetDevice(prev) != cudaSuccess) cudaGetLastError(); }
     DeviceScope(const DeviceScope&) = delete;
     DeviceScope& operator=(const DeviceScope&) = delete;
 };
@@ -126,6 +135,11 @@ int fail(tdse_ctx* ctx, int code, const std::string& msg)
         if (e__ != cudaSuccess)                                                               \
             return fail(ctx, TDSE_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e__)); \
     } while (0)
+
+#define ENTER_DEVICE(ctx)                                                                          \
+    DeviceScope on_device_(ctx);                                                                   \
+    if (!on_device_.ok())                                                                          \
+        return fail(ctx, TDSE_ECUDA, std::string("cannot make the context's device current: ") + cudaGetErrorString(on_device_.err))
 
 #define CU_LAUNCH_CHECK(ctx)                                                                     \
     do {                                                                                         \
@@ -352,10 +366,12 @@ int launch_fused_cfg(tdse_ctx* c, FusedParams& P, int ctas_per_sm = MINB)
     auto kern = fdtd_fused_kernel<real, T, BX, BY, NT, PF, GHOSTXY, MINB, SPLIT>;
     constexpr size_t kMaxSmem = MINB == 1 ? 227 * 1024 : (228 * 1024) / MINB - 1024;   // per CTA (1 KB reserved each)
     static_assert(Tr::SMEM_FIXED + 64 * sizeof(real) <= kMaxSmem, "fused tile does not fit in shared memory");
-    static bool attr_set[kMaxDevices] = {};          // the attribute is per device, not per process
-    if (c->device >= kMaxDevices || !attr_set[c->device]) {
+    // the attribute is per device, not per process; contexts on several host threads may get here together (setting it
+    // twice is harmless, the flag only saves the call)
+    static std::atomic<bool> attr_set[kMaxDevices];
+    if (c->device >= kMaxDevices || !attr_set[c->device].load(std::memory_order_acquire)) {
         CU_TRY(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMaxSmem));
-        if (c->device < kMaxDevices) attr_set[c->device] = true;
+        if (c->device < kMaxDevices) attr_set[c->device].store(true, std::memory_order_release);
     }
     int rc = plan_fused<real, T, BX, BY, NT, PF, MINB>(c, ctas_per_sm, &P.tiles_x, &P.tiles_y, &P.bz, &P.nchunks, nullptr);
     if (rc) return rc;
@@ -489,12 +505,13 @@ int launch_twopass_step(tdse_ctx* c)
 
 // Streamed frame mode: the ring slot the next frame goes to (NULL once the host buffer is full).  The compute stream first
 // waits until the copy that last used this slot has left it.
-int stream_frame_begin(tdse_ctx* c, double** frame)
+int stream_frame_begin(tdse_ctx* c, double** frame, bool* waited)
 {
     *frame = nullptr;
+    *waited = false;
     if (c->nframes >= c->fs_capacity) return TDSE_OK;
     const int slot = c->nframes % c->fs_slots;
-    if (c->fs_busy[slot]) CU_TRY(c, cudaStreamWaitEvent(c->stream, c->fs_copied[slot], 0));
+    if (c->fs_busy[slot]) { CU_TRY(c, cudaStreamWaitEvent(c->stream, c->fs_copied[slot], 0)); *waited = true; }
     *frame = c->fs_ring + (size_t)slot * c->g.batch * c->g.plane;
     return TDSE_OK;
 }
@@ -508,8 +525,14 @@ int stream_frame_end(tdse_ctx* c, double* frame)
         const size_t plane_bytes = (size_t)c->g.plane * sizeof(double);
         CU_TRY(c, cudaEventRecord(c->fs_written[slot], c->stream));
         CU_TRY(c, cudaStreamWaitEvent(c->fs_stream, c->fs_written[slot], 0));
-        CU_TRY(c, cudaMemcpy2DAsync(c->fs_host + (size_t)c->nframes * c->g.plane, (size_t)c->fs_capacity * plane_bytes, frame, plane_bytes,
-                                    plane_bytes, (size_t)c->g.batch, cudaMemcpyDeviceToHost, c->fs_stream));
+        if (c->fs_copy2d) {
+            CU_TRY(c, cudaMemcpy2DAsync(c->fs_host + (size_t)c->nframes * c->g.plane, (size_t)c->fs_capacity * plane_bytes, frame, plane_bytes,
+                                        plane_bytes, (size_t)c->g.batch, cudaMemcpyDeviceToHost, c->fs_stream));
+        } else {      // host pitch capacity * plane beyond what a 2-D copy takes (cudaDevAttrMaxPitch): one copy per entry
+            for (int b = 0; b < c->g.batch; ++b)
+                CU_TRY(c, cudaMemcpyAsync(c->fs_host + ((size_t)b * c->fs_capacity + c->nframes) * c->g.plane, frame + (size_t)b * c->g.plane,
+                                          plane_bytes, cudaMemcpyDeviceToHost, c->fs_stream));
+        }
         CU_TRY(c, cudaEventRecord(c->fs_copied[slot], c->fs_stream));
         c->fs_busy[slot] = 1;
     }
@@ -531,14 +554,17 @@ void free_frame_stream(tdse_ctx* c)
 
 // one launch per sample (accumulate + trace), programmatically serialised behind the step kernel
 template <typename real>
-int launch_detector(tdse_ctx* c, double* D, double* partial, double* frame, long long frame_entry_stride, int slot)
+int launch_detector(tdse_ctx* c, double* D, double* partial, double* frame, long long frame_entry_stride, int slot,
+                    bool allow_pdl = true)
 {
     const unsigned nblk = (unsigned)((c->g.plane + 255) / 256);
     cudaLaunchConfig_t lc = {};
     lc.gridDim = dim3(nblk, (unsigned)c->g.batch); lc.blockDim = dim3(256); lc.dynamicSmemBytes = 0; lc.stream = c->stream;
     cudaLaunchAttribute la[1];
     la[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    la[0].val.programmaticStreamSerializationAllowed = c->opt_pdl ? 1 : 0;
+    // griddepcontrol.wait orders this kernel behind the preceding KERNEL only.  When the stream has just been told to wait
+    // for a ring slot's copy-out event, the launch must be a plain, fully stream-ordered one: nothing may touch the slot early.
+    la[0].val.programmaticStreamSerializationAllowed = (c->opt_pdl && allow_pdl) ? 1 : 0;
     lc.attrs = la; lc.numAttrs = 1;
     CU_TRY(c, cudaLaunchKernelEx(&lc, detector_accum_kernel<real>, c->g, c->k_det, static_cast<const real*>(c->R[c->cur]),
                                  static_cast<const real*>(c->I[c->cur]), D, partial, frame, frame_entry_stride,
@@ -559,9 +585,10 @@ int sample_detector(tdse_ctx* c)
     }
     if (c->fs_ring) {
         double* frame = nullptr;
-        rc = stream_frame_begin(c, &frame);
+        bool waited = false;
+        rc = stream_frame_begin(c, &frame, &waited);
         if (rc) return rc;
-        rc = launch_detector<real>(c, c->D, c->partial, frame, c->g.plane, c->nsamples);
+        rc = launch_detector<real>(c, c->D, c->partial, frame, c->g.plane, c->nsamples, !waited);
         if (rc) return rc;
         if ((rc = stream_frame_end(c, frame))) return rc;
     } else {
@@ -580,9 +607,10 @@ int sample_initial_frame(tdse_ctx* c)
 {
     if (c->fs_ring) {
         double* frame = nullptr;
-        int rc = stream_frame_begin(c, &frame);
+        bool waited = false;
+        int rc = stream_frame_begin(c, &frame, &waited);
         if (rc) return rc;
-        if ((rc = launch_detector<real>(c, nullptr, nullptr, frame, c->g.plane, 0))) return rc;
+        if ((rc = launch_detector<real>(c, nullptr, nullptr, frame, c->g.plane, 0, !waited))) return rc;
         return stream_frame_end(c, frame);
     }
     const int rc = launch_detector<real>(c, nullptr, nullptr, c->frames, (long long)c->max_frames * c->g.plane, 0);
@@ -638,13 +666,13 @@ int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
     c->arr_bytes = align_up((size_t)c->g.pcells * batch * c->w);
     c->have_V.assign(batch, 0);
     c->have_state.assign(batch, 0);
-    cudaGetDevice(&c->device);
-    cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
     auto bail = [&](const char* what, cudaError_t err) {
         std::string m = std::string("tdse_create: ") + what + ": " + cudaGetErrorString(err);
         tdse_destroy(c);
         return fail(nullptr, TDSE_ECUDA, m);
     };
+    if ((e = cudaGetDevice(&c->device)) != cudaSuccess) return bail("cudaGetDevice", e);
+    if ((e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device)) != cudaSuccess) return bail("SM count", e);
     if ((e = cudaMalloc(&c->D, (size_t)batch * c->g.plane * sizeof(double))) != cudaSuccess) return bail("detector image", e);
     if ((e = cudaMalloc(&c->scalars, 4 * sizeof(double))) != cudaSuccess) return bail("scalars", e);
     if ((e = cudaEventCreateWithFlags(&c->atoms_ev, cudaEventDisableTiming)) != cudaSuccess) return bail("event", e);
@@ -659,7 +687,7 @@ int tdse_create(tdse_ctx** out, int nx, int ny, int nz, int batch,
 int tdse_destroy(tdse_ctx* c)
 {
     if (!c) return TDSE_OK;
-    DeviceScope on_device_(c);
+    DeviceScope on_device_(c);      // frees what it can even if the switch failed
     cudaStreamSynchronize(c->stream);
     if (c->ws_owned && c->ws) cudaFree(c->ws);
     if (c->mask_dev) cudaFree(c->mask_dev);
@@ -685,7 +713,7 @@ int tdse_destroy(tdse_ctx* c)
 int tdse_bind(tdse_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (!dev_workspace) return fail(c, TDSE_EINVAL, "tdse_bind: workspace is NULL");
     if (reinterpret_cast<uintptr_t>(dev_workspace) % kAlign) return fail(c, TDSE_EINVAL, "tdse_bind: workspace must be 256-byte aligned");
     if (bytes < 3 * c->arr_bytes) return fail(c, TDSE_ENOMEM, "tdse_bind: workspace smaller than tdse_workspace_bytes(..., 0)");
@@ -702,7 +730,7 @@ int tdse_bind(tdse_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream)
 int tdse_set_boundary(tdse_ctx* c, int bcx, int bcy, int bcz, int absorb_lo, int absorb_hi, double strength, int power)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     auto okbc = [](int b) { return b == TDSE_BC_PERIODIC || b == TDSE_BC_DIRICHLET; };
     if (!okbc(bcx) || !okbc(bcy) || !okbc(bcz)) return fail(c, TDSE_EINVAL, "tdse_set_boundary: unknown boundary flag");
     if (absorb_lo < 0 || absorb_hi < 0 || absorb_lo + absorb_hi > c->g.nz) return fail(c, TDSE_EINVAL, "tdse_set_boundary: absorber widths");
@@ -843,7 +871,7 @@ extern "C" {
 int tdse_set_spacing(tdse_ctx* c, double dy, double dz)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (!(dy > 0) || !(dz > 0)) return fail(c, TDSE_EINVAL, "tdse_set_spacing: dy, dz must be > 0");
     c->m.dy = dy; c->m.dz = dz;
     c->m.cy = c->hbar * c->dt / (2.0 * c->mass * dy * dy);
@@ -858,7 +886,7 @@ int tdse_set_spacing(tdse_ctx* c, double dy, double dz)
 int tdse_set_potential(tdse_ctx* c, int b, const tdse_atom* atoms_host, int natoms, double vmin, double vmax, double rcut)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (natoms < 0 || (natoms > 0 && !atoms_host)) return fail(c, TDSE_EINVAL, "tdse_set_potential: atom list");
     if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential: vmin > vmax");
     int rc = ensure_workspace(c);
@@ -871,7 +899,7 @@ int tdse_set_potential(tdse_ctx* c, int b, const tdse_atom* atoms_host, int nato
 int tdse_set_potential_device(tdse_ctx* c, int b, const tdse_atom* atoms_device, int natoms, double vmin, double vmax, double rcut)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (natoms < 0 || (natoms > 0 && !atoms_device)) return fail(c, TDSE_EINVAL, "tdse_set_potential_device: atom list");
     if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential_device: vmin > vmax");
     int rc = ensure_workspace(c);
@@ -883,7 +911,7 @@ int tdse_set_potential_batch(tdse_ctx* c, const tdse_atom* atoms, const int* off
                              double vmin, double vmax, double rcut)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     const int batch = c->g.batch;
     if (!offsets_host) return fail(c, TDSE_EINVAL, "tdse_set_potential_batch: offsets is NULL");
     if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential_batch: vmin > vmax");
@@ -930,7 +958,7 @@ int tdse_set_potential_cell(tdse_ctx* c, int b, const double* cell, int on_devic
                             double ax, double ay, double az, double x0, double y0, double z0, double vmin, double vmax)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (!cell || mx < 1 || my < 1 || mz < 1) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: cell grid");
     if (!(ax > 0) || !(ay > 0) || !(az > 0)) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: cell edge lengths must be > 0");
     if (!(vmin <= vmax)) return fail(c, TDSE_EINVAL, "tdse_set_potential_cell: vmin > vmax");
@@ -971,7 +999,7 @@ int tdse_set_potential_cell(tdse_ctx* c, int b, const double* cell, int on_devic
 int tdse_set_potential_grid(tdse_ctx* c, int b, const void* V, int on_device)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (!V) return fail(c, TDSE_EINVAL, "tdse_set_potential_grid: V is NULL");
     int b0, b1;
     if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_potential_grid: entry out of range");
@@ -1003,7 +1031,7 @@ int tdse_set_wavepacket(tdse_ctx* c, int b, double x0, double y0, double z0, dou
                         double kx, double ky, double kz, double amplitude)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (!(sigma > 0)) return fail(c, TDSE_EINVAL, "tdse_set_wavepacket: sigma must be > 0");
     int b0, b1;
     if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_wavepacket: entry out of range");
@@ -1031,7 +1059,7 @@ int tdse_set_wavepacket(tdse_ctx* c, int b, double x0, double y0, double z0, dou
 int tdse_set_state(tdse_ctx* c, int b, const void* R, const void* I_half, int on_device)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (!R || !I_half) return fail(c, TDSE_EINVAL, "tdse_set_state: NULL state");
     int b0, b1;
     if (!entry_range(c, b, &b0, &b1)) return fail(c, TDSE_EINVAL, "tdse_set_state: entry out of range");
@@ -1052,7 +1080,7 @@ int tdse_set_state(tdse_ctx* c, int b, const void* R, const void* I_half, int on
 int tdse_set_detector(tdse_ctx* c, int k_plane, int every, int max_samples)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (every < 0 || max_samples < 0) return fail(c, TDSE_EINVAL, "tdse_set_detector: every, max_samples must be >= 0");
     if (every > 0 && (k_plane < 0 || k_plane >= c->g.nz)) return fail(c, TDSE_EINVAL, "tdse_set_detector: plane out of range");
     if (max_samples != c->max_samples) {
@@ -1076,7 +1104,7 @@ int tdse_set_detector(tdse_ctx* c, int k_plane, int every, int max_samples)
 int tdse_step(tdse_ctx* c, int n)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (n < 0) return fail(c, TDSE_EINVAL, "tdse_step: n < 0");
     if (!c->ws) return fail(c, TDSE_ESTATE, "tdse_step: potential and state are not set");
     for (int e = 0; e < c->g.batch; ++e)
@@ -1142,7 +1170,7 @@ int tdse_step(tdse_ctx* c, int n)
 int tdse_detector_read(tdse_ctx* c, int b, double* image_host, double* trace_host, int cap, int* nsamples)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_detector_read: entry out of range");
     if (cap < 0) return fail(c, TDSE_EINVAL, "tdse_detector_read: cap < 0");
     if (image_host)
@@ -1158,7 +1186,7 @@ int tdse_detector_read(tdse_ctx* c, int b, double* image_host, double* trace_hos
 int tdse_set_frames(tdse_ctx* c, int max_frames, int include_t0)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (max_frames < 0) return fail(c, TDSE_EINVAL, "tdse_set_frames: max_frames < 0");
     CU_TRY(c, cudaStreamSynchronize(c->stream));
     free_frame_stream(c);                // flat and streamed frame mode exclude each other
@@ -1175,7 +1203,7 @@ int tdse_set_frames(tdse_ctx* c, int max_frames, int include_t0)
 int tdse_frames_read(tdse_ctx* c, int b, int first, int count, double* frames_host, int* nframes)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_frames_read: entry out of range");
     const int have = std::min(c->nframes, c->max_frames);
     if (first < 0 || count < 0 || first + count > have) return fail(c, TDSE_EINVAL, "tdse_frames_read: frame range exceeds the frames kept");
@@ -1201,7 +1229,7 @@ int tdse_frames_device(tdse_ctx* c, double** frames_device, int* max_frames, int
 int tdse_set_frame_stream(tdse_ctx* c, double* frames_host, int capacity, int ring_slots, int include_t0)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (capacity < 0 || ring_slots < 0) return fail(c, TDSE_EINVAL, "tdse_set_frame_stream: capacity, ring_slots must be >= 0");
     if (capacity > 0 && (!frames_host || ring_slots < 2)) return fail(c, TDSE_EINVAL, "tdse_set_frame_stream: needs a host buffer and at least 2 ring slots");
     CU_TRY(c, cudaStreamSynchronize(c->stream));
@@ -1222,6 +1250,9 @@ int tdse_set_frame_stream(tdse_ctx* c, double* frames_host, int capacity, int ri
             }
         }
         c->fs_host = frames_host; c->fs_slots = ring_slots; c->fs_capacity = capacity;
+        int max_pitch = 0;
+        if (cudaDeviceGetAttribute(&max_pitch, cudaDevAttrMaxPitch, c->device) != cudaSuccess) { cudaGetLastError(); max_pitch = 0; }
+        c->fs_copy2d = (size_t)capacity * c->g.plane * sizeof(double) <= (size_t)std::max(max_pitch, 0);
     }
     return reset_detector(c);
 }
@@ -1229,7 +1260,7 @@ int tdse_set_frame_stream(tdse_ctx* c, double* frames_host, int capacity, int ri
 int tdse_frames_sync(tdse_ctx* c, int* nframes)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (!c->fs_ring) return fail(c, TDSE_ESTATE, "tdse_frames_sync: streamed frame mode is off (tdse_set_frame_stream)");
     CU_TRY(c, cudaStreamSynchronize(c->stream));       // every sample has been launched and has handed its slot over ...
     CU_TRY(c, cudaStreamSynchronize(c->fs_stream));    // ... and every copy has landed
@@ -1240,7 +1271,7 @@ int tdse_frames_sync(tdse_ctx* c, int* nframes)
 int tdse_dissimilarity(tdse_ctx* c, int first_frame, int last_frame, double* d_host)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (!d_host) return fail(c, TDSE_EINVAL, "tdse_dissimilarity: NULL");
     if (!c->frames) return fail(c, TDSE_ESTATE, "tdse_dissimilarity: frame mode is off (tdse_set_frames)");
     const int have = std::min(c->nframes, c->max_frames);
@@ -1274,7 +1305,7 @@ int tdse_detector_device(tdse_ctx* c, double** image_device, double** trace_devi
 int tdse_read_psi(tdse_ctx* c, int b, void* R_host, void* I_host)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_read_psi: entry out of range");
     if (!c->ws || !c->have_state[b]) return fail(c, TDSE_ESTATE, "tdse_read_psi: state not set");
     int rc;
@@ -1287,7 +1318,7 @@ int tdse_read_psi(tdse_ctx* c, int b, void* R_host, void* I_host)
 int tdse_read_potential(tdse_ctx* c, int b, void* V_host)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_read_potential: entry out of range");
     if (!c->ws || !c->have_V[b]) return fail(c, TDSE_ESTATE, "tdse_read_potential: potential not set");
     if (!V_host) return fail(c, TDSE_EINVAL, "tdse_read_potential: NULL");
@@ -1299,7 +1330,7 @@ int tdse_read_potential(tdse_ctx* c, int b, void* V_host)
 int tdse_norm(tdse_ctx* c, int b, double* q_visscher, double* q_paper)
 {
     if (!c) return TDSE_EINVAL;
-    DeviceScope on_device_(c);
+    ENTER_DEVICE(c);
     if (b < 0 || b >= c->g.batch) return fail(c, TDSE_EINVAL, "tdse_norm: entry out of range");
     if (!c->ws || !c->have_state[b] || !c->have_V[b]) return fail(c, TDSE_ESTATE, "tdse_norm: potential and state must be set");
     const unsigned nblk = (unsigned)((c->g.cells + 255) / 256);

@@ -54,10 +54,14 @@ __device__ __forceinline__ double sqrt_pos(double a)
 // exp(x) = 2^(n div 256) * T[n mod 256] * (1 + q(r)), q = expm1 as a degree-4 polynomial (remainder r^5/120 < 4e-17).
 // r comes from one fma with ln2/256 rounded to double: its error, |n| * 2^-61, stays below 2e-15 for every term that
 // is not itself below 1e-16 (|x| < 37).  Below x = -708 the result stays near 2^-1022, which no sum registers.  exp(-0) = 1.
+// x is clamped at -746 first (one DMNMX): a screening length far below the mesh (or a denormal one, inv_screen = inf)
+// gives x = -1e10 or -inf, where the integer n would wrap and r = inf - inf; the clamp turns those into "about 2^-1022",
+// which is what exp underflows to.  Every x > -746 goes through unchanged.
 constexpr int kExpTable = 256;
 
 __device__ __forceinline__ double exp_nonpositive(double x, const double* __restrict__ T)
 {
+    x = fmax(x, -746.0);
     double t = fma(x, (double)kExpTable * 1.4426950408889634074, kRoundMagic);
     const int n = max(__double2loint(t), -1022 * kExpTable);        // n = 256 k + j; k >= -1022 keeps the result a normal number
     t -= kRoundMagic;
