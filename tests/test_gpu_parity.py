@@ -487,6 +487,76 @@ def test_flat_offsets_beyond_2_31_elements_per_array():
     t.close()
 
 
+@pytest.mark.skipif(bool(os.environ.get("TDSE_SKIP_FULL_PARITY")), reason="TDSE_SKIP_FULL_PARITY set (minutes of oracle time)")
+def test_detector_plane_in_the_rounding_noise_is_no_worse_than_the_float_oracle():
+    """The geometry DESIGN.md reading 19 retired (round 1's literal cfg 4: packet at 0.3 Lz, slab top at 0.6 Lz, detector plane
+    k = 10), kept as a noise-floor case on a 64 x 64 x 512 column that preserves the distances along z: the plane sits 5.4 sigma
+    behind the packet and sees, within 2000 steps, only the Gaussian tail (1e-12 of the peak density) and the float rounding
+    noise the packet radiates.  The 1e-4 image tolerance cannot be met there by ANY float code -- the oracle's own float
+    instantiation misses its fp64 run by 5.7e-3 -- so the claim tested is: the GPU's image error is within 2x of that floor,
+    while psi itself still meets 1e-4."""
+    from paper_2401_07416_b200 import Tdse
+    from workloads.configs import fcc111_slab
+    w = make_config(4, n=(64, 64, 512), dtype="f32", batch=1)
+    lx, ly, lz = w.nx * w.dx, w.ny * w.dx, w.nz * w.dx
+    pk = dict(w.packet)
+    pk["z0"] = 0.3 * lz
+    w = w.with_(atoms=[fcc111_slab(lx, ly, 0.6 * lz, 4)], packet=pk, k_det=10)
+    assert (pk["z0"] - w.k_det * w.dx) / pk["sigma"] > 5.0 and w.steps == 2000
+    t = Tdse.from_workload(w)
+    t.step(w.steps)
+    R, I = t.read_psi(0)
+    D, tr = t.detector_read(0)
+    t.close()
+    o64 = OracleRun.from_workload(w, dtype="f64", round_to="f32").step(w.steps)
+    o32 = OracleRun.from_workload(w, dtype="f32").step(w.steps)
+    e_gpu, e_orc = rel_l2(D, o64.D), rel_l2(o32.D, o64.D)
+    print("noise-floor plane: image rel-L2 GPU f32 vs oracle f64 %.3e, oracle f32 vs oracle f64 %.3e; psi GPU %.3e, oracle f32 %.3e"
+          % (e_gpu, e_orc, rel_l2(R, o64.R), rel_l2(o32.R, o64.R)))
+    assert e_orc > 1e-4                                   # the float floor itself is above the tolerance here
+    assert e_gpu <= 2.0 * e_orc
+    assert rel_l2(R, o64.R) < 1e-4 and rel_l2(I, o64.I) < 1e-4
+
+
+@pytest.mark.skipif(bool(os.environ.get("TDSE_SKIP_FULL_PARITY")), reason="TDSE_SKIP_FULL_PARITY set (minutes of oracle time)")
+@pytest.mark.parametrize("dtype,batch", [("f64", 48), ("f32", 40)])
+def test_config4_at_the_batch_that_fills_hbm_first_and_last_entry(dtype, batch):
+    """BASELINE.json configs[4] is the batch "scaled to fill most of the 180 GB": 40 x 512^3 f32 / 48 x 384^3 f64 are
+    111 / 113 GB of workspace, the launch shape (grid size, wave count, entry offsets far beyond 2^31 elements) of the
+    fill-HBM runs BASELINE.md quotes.  SURVEY.md section 8(d): the oracle runs entries 0 and batch-1, the rest is covered
+    by position invariance.  Entry 0 is the undisplaced slab, entry batch-1 a thermally displaced one (seed 4000 + b,
+    workloads/configs.py); both are compared with the oracle in every cell after 20 steps (two detector samples), with
+    the per-cell guard; entry 17 is a planted copy of entry batch-1 and must equal it bit for bit."""
+    import torch
+    from paper_2401_07416_b200 import Tdse
+    w = make_config(4, dtype=dtype, batch=batch, steps=20)
+    assert (w.nx, w.batch, w.every) == (512 if dtype == "f32" else 384, batch, 10)
+    assert w.seeds[0] is None and w.seeds[batch - 1] == 4000 + batch - 1
+    atoms = list(w.atoms)
+    atoms[17] = atoms[batch - 1].copy()
+    w = w.with_(atoms=atoms)
+    t = Tdse.from_workload(w)
+    assert t.workspace.numel() > 100e9
+    t.step(w.steps)
+    assert (t.get_info("kernel"), t.get_info("tblock")) == (FUSED, 2)
+    out = {b: t.read_psi(b) + t.detector_read(b) for b in (0, 17, batch - 1)}
+    t.close()
+    del t
+    torch.cuda.empty_cache()                      # hand the 110 GB back before the next test's context
+    for x17, xl in zip(out[17], out[batch - 1]):
+        assert np.array_equal(x17, xl)
+    for b in (0, batch - 1):
+        R, I, D, tr = out[b]
+        o = oracle_for(w, b, w.steps)
+        assert len(tr) == len(o.trace) == 2
+        errs = (rel_l2(R, o.R), rel_l2(I, o.I), rel_l2(D, o.D), rel_l2(tr, o.trace))
+        cell = max(max_abs_rel(R, o.R), max_abs_rel(I, o.I), max_abs_rel(D, o.D))
+        print("fill-HBM parity cfg4 %s %d x %d^3, entry %d, %d steps: rel-L2 R %.3e I %.3e D %.3e trace %.3e, per-cell %.3e"
+              % (dtype, batch, w.nx, b, w.steps, *errs, cell))
+        assert max(errs) < TOL[dtype] and cell < CELL_TOL[dtype], "entry %d" % b
+    assert not np.array_equal(out[0][0], out[batch - 1][0])        # the displaced entry really differs
+
+
 # ------------------------------------------------------------------------------------------
 # frame-mode detector (PAPER.md:158-162) and pairwise dissimilarity (eq 16, PAPER.md:219-221)
 # ------------------------------------------------------------------------------------------
@@ -792,6 +862,34 @@ def test_atoms_many_periods_outside_the_box_with_a_cutoff():
     assert np.max(np.abs(o.V64 - o_in.V64)) <= 1e-9 * np.max(np.abs(o_in.V64))     # the shifted list is the same crystal
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("rcut", [0.0, 3.07])     # not a multiple of dx: with an atom ON a grid point, cells at lattice distances
+def test_screening_lengths_far_below_the_mesh_and_denormal(dtype, rcut):   # (12, 16, 0) dx = 20 dx would sit exactly on the cutoff, where keep / skip hangs on the last bit of r^2
+    """exp(-r/screen) with screen = 1e-8 (x = -1e10) and a denormal screen (1/screen = inf, x = -inf) underflows to 0 in
+    the definition (include/tdse.h; libm in the oracle).  The builder's table exp must do the same instead of wrapping
+    its integer exponent or producing inf - inf: those atoms contribute nothing, the others are unaffected."""
+    from paper_2401_07416_b200 import Tdse
+    w = make_config(4, n=(48, 40, 56), batch=1, dtype=dtype)
+    atoms = w.atoms[0].copy()
+    atoms[:, 0:3] += np.array([0.0123, 0.0077, 0.0031]) * w.dx     # no screened atom sits exactly on a grid point (r = 0)
+    atoms[0::4, 5] = 1e-8          # column 5 = screen
+    atoms[1::4, 5] = 5e-324        # smallest denormal
+    atoms[2::4, 5] = 2e-3          # x around -1e3 .. -1e4: below -746, inside the int range
+    atoms[3, 0:3] = (7 * w.dx, 5 * w.dx, 9 * w.dx)     # an unscreened-range atom exactly on a grid point stays finite
+    w2 = w.with_(atoms=[atoms], rcut=rcut)
+    t = Tdse.from_workload(w2)
+    V = t.read_potential(0)
+    t.close()
+    o = OracleRun.from_workload(w2, entry=0, dtype="f64", round_to="f32" if dtype == "f32" else None)
+    assert np.all(np.isfinite(V))
+    if dtype == "f64":
+        assert np.max(np.abs(V - o.V64)) <= 1e-13 * max(1.0, np.max(np.abs(o.V64)))
+    else:
+        ulp = np.spacing(np.abs(o.V).astype(np.float32)).astype(np.float64)
+        assert np.all(np.abs(V.astype(np.float64) - o.V) <= ulp)
+    assert np.ptp(o.V64) > 0.1                                       # the remaining quarter of the atoms still shapes V
+
+
 def test_set_detector_keeps_the_trace_buffer_and_survives_a_failed_allocation():
     from paper_2401_07416_b200 import Tdse, TdseError, TDSE_ENOMEM
     w = make_config(0, n=(24, 24, 24), steps=0, batch=64)
@@ -952,6 +1050,138 @@ def test_streamed_frames_equal_the_flat_frame_mode_bit_for_bit(dtype, include_t0
     for b in range(w.batch):
         assert np.array_equal(again[b], want[b][:cap])
     t.set_frame_stream(0, 0)                               # off
+    t.close()
+
+
+# ------------------------------------------------------------------------------------------
+# the paper's own mesh as ONE pass: unit-cell potential resampled onto 240 x 240 x (420 + 100)
+# anisotropic cells, periodic on all axes with the 100-plane absorber at the bottom, packet moving down, a frame every
+# 20 steps streamed to the host, then eq (16) between the configurations
+# ------------------------------------------------------------------------------------------
+def _paper_ctx(m, **kw):
+    from paper_2401_07416_b200 import Tdse
+    t = Tdse(m.nx, m.ny, m.nz, m.batch, m.dx, m.dt, m.mass, m.hbar, m.dtype, **kw)
+    t.set_spacing(m.dy, m.dz)
+    t.set_boundary(*m.bc, m.absorb_lo, m.absorb_hi, m.strength, m.power)
+    for b in range(m.batch):
+        t.set_potential_cell(b, m.unit_cells[b], m.cell_edges, m.cell_origin, m.vmin, m.vmax)
+    p = m.packet
+    t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
+    return t
+
+
+def _paper_oracle(m, b):
+    o = OracleRun(m.nx, m.ny, m.nz, m.dx, m.dt, m.mass, m.hbar, "f64", m.bc, m.absorb_lo, m.absorb_hi, m.strength, m.power,
+                  round_to="f32" if m.dtype == "f32" else None, dy=m.dy, dz=m.dz)
+    o.set_potential_cell(m.unit_cells[b], m.cell_edges, m.cell_origin, m.vmin, m.vmax)
+    o.set_wavepacket(**m.packet)
+    o.set_detector(m.k_det, m.every)
+    return o.set_frames(True, True)
+
+
+@pytest.mark.parametrize("n,steps,dtype", [((48, 32, 84), 200, "f64"), ((48, 32, 84), 200, "f32"), (None, 300, "f32")])
+def test_paper_mesh_whole_pass_matches_oracle(n, steps, dtype):
+    """n = None is the full 240 x 240 x 520 mesh: nx = 240 is 3.75 of the fused kernel's 64-wide f32 tiles and ny = 240 is 7.5 of
+    its 32 rows, so the ragged last tile column and row run at the size the paper uses.  Entries 0 and batch-1 against the
+    oracle: V, psi, image, trace and every streamed frame; the device-frame run must reproduce the streamed frames bit for
+    bit, and d_kj from it must match eq (16) evaluated by the oracle on the oracle's own frames."""
+    from workloads import paper_mesh
+    m = paper_mesh(batch=3, steps=steps, n=n, dtype=dtype)
+    tol = TOL[dtype]
+    nfr = steps // m.every + 1
+    t = _paper_ctx(m)
+    t.set_detector(m.k_det, m.every, nfr)
+    t.set_frame_stream(nfr, 3, True)
+    t.step(steps)
+    got = t.frames_sync().copy()
+    assert got.shape == (m.batch, nfr, m.ny, m.nx)
+    if n is None:
+        assert (t.get_info("kernel"), t.get_info("tblock"), t.get_info("tile_x"), t.get_info("tile_y")) == (FUSED, 2, 64, 32)
+    ora = {}
+    for b in (0, m.batch - 1):
+        o = _paper_oracle(m, b)
+        V = t.read_potential(b)
+        if dtype == "f64":
+            assert np.max(np.abs(V - o.V64)) <= 1e-13 * max(1.0, np.max(np.abs(o.V64)))
+        else:
+            assert np.all(np.abs(V.astype(np.float64) - o.V) <= np.spacing(np.abs(o.V).astype(np.float32)).astype(np.float64))
+        o.step(steps)
+        R, I = t.read_psi(b)
+        D, tr = t.detector_read(b)
+        errs = (rel_l2(R, o.R), rel_l2(I, o.I), rel_l2(D, o.D), rel_l2(tr, o.trace))
+        cell = max(max_abs_rel(R, o.R), max_abs_rel(I, o.I), max_abs_rel(D, o.D))
+        fr_err = max(rel_l2(got[b][s], o.frames[s]) for s in range(nfr))
+        print("paper mesh %s %dx%dx%d entry %d, %d steps: rel-L2 R %.3e I %.3e D %.3e trace %.3e frames %.3e, per-cell %.3e"
+              % (dtype, m.nx, m.ny, m.nz, b, steps, *errs, fr_err, cell))
+        assert max(errs) < tol and cell < CELL_TOL[dtype] and fr_err < tol and len(o.frames) == nfr
+        ora[b] = np.array(o.frames)
+    # the same trajectories with the frames kept on the device, then eq (16)
+    t.set_frames(nfr, True)
+    p = m.packet
+    t.set_wavepacket(-1, p["x0"], p["y0"], p["z0"], p["sigma"], p["kx"], p["ky"], p["kz"], p["amplitude"])
+    t.step(steps)
+    for b in range(m.batch):
+        assert np.array_equal(t.frames_read(b), got[b])
+    d = t.dissimilarity(1, nfr - 1)
+    want = oracle.dissimilarity(ora[0], ora[m.batch - 1], m.dx * m.dy, 1, nfr - 1)
+    assert want > 0 and abs(d[0, m.batch - 1] - want) <= 10 * tol * want
+    t.close()
+
+
+def _random_ctx(nx, ny, nz, batch, dtype, seed):
+    t = make_ctx(nx, ny, nz, batch, 0.25, 0.004, dtype)
+    t.set_boundary(PERIODIC, PERIODIC, DIRICHLET, 2, 2, 0.07, 2)
+    for b in range(batch):
+        V = random_potential(seed + b, (nz, ny, nx), -30.0, 5.0)
+        R0, I0 = random_state(seed + 100 + b, (nz, ny, nx))
+        t.set_potential_grid(b, V.astype(t.np_dtype))
+        t.set_state(b, R0.astype(t.np_dtype), I0.astype(t.np_dtype))
+    return t
+
+
+@pytest.mark.parametrize("pinned", [True, False])
+def test_streamed_frames_ring_of_two_sampled_every_step_on_large_planes(pinned):
+    """The hard case for slot reuse: a sample after EVERY step, only two ring slots, 2 MiB per entry and frame (512 x 512),
+    so the step that comes back to a slot finds its copy-out still under way (always with a pageable host buffer, where
+    the copies serialise; usually with a pinned one).  The detector launch that follows the wait on the slot's event is
+    a plain stream-ordered launch (no programmatic dependent launch), and every frame must equal the flat mode's."""
+    nx, ny, nz, batch, steps = 512, 512, 12, 2, 24
+    flat = _random_ctx(nx, ny, nz, batch, "f32", 900)
+    flat.set_detector(5, 1, steps)
+    flat.set_frames(steps + 1, True)
+    flat.step(steps)
+    want = [flat.frames_read(b) for b in range(batch)]
+    flat.close()
+    t = _random_ctx(nx, ny, nz, batch, "f32", 900)
+    t.set_detector(5, 1, steps)
+    t.set_frame_stream(steps + 1, 2, True, pinned=pinned)
+    t.step(steps)
+    got = t.frames_sync()
+    assert got.shape == (batch, steps + 1, ny, nx)
+    for b in range(batch):
+        assert np.array_equal(got[b], want[b]), "entry %d" % b
+    t.close()
+
+
+def test_streamed_frames_with_a_host_pitch_beyond_the_2d_copy_limit():
+    """capacity * ny * nx * 8 bytes = 257 * 8 MiB > 2^31 - 1 (cudaDevAttrMaxPitch): the strided 2-D copy cannot carry that
+    pitch, so a slot leaves as one copy per entry.  Same frames as the flat mode, at the right places of the host buffer
+    (only the few frames taken are ever touched in the 4 GiB pageable buffer)."""
+    nx, ny, nz, batch, steps, cap = 1024, 1024, 8, 2, 3, 257
+    flat = _random_ctx(nx, ny, nz, batch, "f32", 950)
+    flat.set_detector(3, 1, steps)
+    flat.set_frames(steps + 1, True)
+    flat.step(steps)
+    want = [flat.frames_read(b) for b in range(batch)]
+    flat.close()
+    t = _random_ctx(nx, ny, nz, batch, "f32", 950)
+    t.set_detector(3, 1, steps)
+    t.set_frame_stream(cap, 2, True, pinned=False)
+    t.step(steps)
+    got = t.frames_sync()
+    assert got.shape == (batch, steps + 1, ny, nx)
+    for b in range(batch):
+        assert np.array_equal(got[b], want[b]), "entry %d" % b
     t.close()
 
 

@@ -11,7 +11,7 @@ The inputs stand in for the paper's Cu(111) and Au(111)/C6-SAM workloads
 available; see DESIGN.md "Input recipe".
 """
 from .configs import (Workload, make_config, fcc111_slab, molecule_template, CONFIG_NAMES,
-                      random_state, random_potential, shard_for_rank, PERIODIC, DIRICHLET)
+                      random_state, random_potential, shard_for_rank, PERIODIC, DIRICHLET, PaperMesh, paper_mesh)
 
 __all__ = ["Workload", "make_config", "fcc111_slab", "molecule_template", "CONFIG_NAMES",
-           "random_state", "random_potential", "shard_for_rank", "PERIODIC", "DIRICHLET"]
+           "random_state", "random_potential", "shard_for_rank", "PERIODIC", "DIRICHLET", "PaperMesh", "paper_mesh"]

@@ -292,3 +292,94 @@ def random_state(seed: int, shape: Sequence[int], dtype=np.float64) -> Tuple[np.
 def random_potential(seed: int, shape: Sequence[int], lo: float, hi: float, dtype=np.float64) -> np.ndarray:
     rng = np.random.default_rng(seed)
     return rng.uniform(lo, hi, size=tuple(shape)).astype(dtype)
+
+
+# ------------------------------------------------------------------------------------------------
+# The paper's own mesh (section 2.3), as inputs only: sizes, spacings, a synthetic unit-cell
+# potential per configuration, packet and detector parameters.  Stands in for the DFT potentials, which are not available.
+# ------------------------------------------------------------------------------------------------
+BOHR_PER_ANGSTROM = 1.0 / 0.529177210903
+HARTREE_PER_EV = 1.0 / 27.211386245988
+
+
+@dataclass
+class PaperMesh:
+    name: str
+    nx: int
+    ny: int
+    nz: int                         # 420 cell planes + 100 absorber planes appended below
+    batch: int
+    dtype: str
+    dx: float
+    dy: float
+    dz: float
+    dt: float                       # eq (11)
+    bc: Tuple[int, int, int]        # periodic on all three axes
+    absorb_lo: int                  # 100 planes at the bottom, none at the top
+    absorb_hi: int
+    strength: float
+    power: int
+    cells_mz_my_mx: Tuple[int, int, int]
+    cell_edges: Tuple[float, float, float]
+    cell_origin: Tuple[float, float, float]
+    unit_cells: List[np.ndarray]    # one [mz][my][mx] float64 grid per configuration
+    vmin: float
+    vmax: float
+    packet: dict
+    k_det: int
+    every: int                      # h = 20
+    steps: int                      # 5000
+    mass: float = 1.0
+    hbar: float = 1.0
+
+    @property
+    def cells(self) -> int:
+        return self.nx * self.ny * self.nz
+
+
+def paper_mesh(batch: int = 8, steps: int = 5000, n: Optional[Sequence[int]] = None, seed: int = 5000,
+               dtype: str = "f32") -> PaperMesh:
+    """240 x 240 x (420 + 100) points on the 35.4 x 40.9 x 70.0 Angstrom domain: anisotropic spacings,
+    a 16 x 16 x 420 unit cell repeated 15 x 15 times in x and y, a 100-plane absorber appended below the cell, periodic
+    on all axes; packet above the surface at r_z = 42.0 A moving down with E = 60 eV, sigma = 1.8 A (PAPER.md:148);
+    detector plane at z_det = 37.6 A, a frame every h = 20 steps; 5000 steps (the data-set runs).
+    `n` = (nx, ny, nz_cell) shrinks the mesh for tests (nx, ny multiples of 16; the absorber keeps nz_cell * 100 // 420 planes).
+    The unit-cell potential is synthetic: four attractive atomic layers below 28.35 A with a lateral corrugation, plus a
+    seeded smooth bump per configuration above the top layer (standing in for one C6-SAM orientation)."""
+    nx, ny, nzc = n or (240, 240, 420)
+    assert nx % 16 == 0 and ny % 16 == 0
+    nabs = 100 * nzc // 420
+    A = BOHR_PER_ANGSTROM
+    dx, dy, dz = 35.4 * A / 240, 40.9 * A / 240, 70.0 * A / 420
+    mx, my, mz = 16, 16, nzc
+    ax, ay, az = mx * dx, my * dy, (mz - 1) * dz
+    zs = np.arange(mz) * dz                                   # heights above the bottom of the cell
+    scale = nzc / 420.0                                       # reduced meshes keep the proportions along z
+    z_top = 28.35 * A * scale
+    xs, ys = np.arange(mx) / mx, np.arange(my) / my
+    corr = 1.0 + 0.3 * np.cos(2 * np.pi * xs)[None, None, :] * np.cos(2 * np.pi * ys)[None, :, None]
+    base = np.zeros((mz, my, mx))
+    for layer in range(4):
+        zc = z_top - layer * 2.08 * A * scale
+        base += -18.0 * np.exp(-0.5 * ((zs - zc) / (0.45 * A * scale)) ** 2)[:, None, None] * corr
+    cells = []
+    for b in range(batch):
+        rng = np.random.default_rng(seed + b)
+        cx, cy = rng.uniform(0, 1, 2)
+        zc = z_top + rng.uniform(1.0, 6.0) * A * scale
+        bump = (-6.0 * np.exp(-0.5 * ((zs - zc) / (1.2 * A * scale)) ** 2)[:, None, None]
+                * (1.0 + 0.8 * np.cos(2 * np.pi * (xs - cx))[None, None, :] * np.cos(2 * np.pi * (ys - cy))[None, :, None]))
+        cells.append(np.ascontiguousarray(base + bump))
+    energy = 60.0 * HARTREE_PER_EV
+    k = math.sqrt(2.0 * energy)                               # = 2 pi / lambda of eq (4), PAPER.md:56 (hbar = m = 1)
+    lx, ly = nx * dx, ny * dy
+    z0 = (nabs + 42.0 / 70.0 * (nzc - 1)) * dz
+    k_det = nabs + int(round(37.6 / 70.0 * (nzc - 1)))
+    return PaperMesh(
+        name="paper_mesh_%dx%dx%d_%s" % (nx, ny, nzc + nabs, dtype), nx=nx, ny=ny, nz=nzc + nabs, batch=batch, dtype=dtype,
+        dx=dx, dy=dy, dz=dz, dt=0.2 * min(dx, dy, dz) ** 2,
+        bc=(PERIODIC, PERIODIC, PERIODIC), absorb_lo=nabs, absorb_hi=0, strength=0.05, power=2,
+        cells_mz_my_mx=(mz, my, mx), cell_edges=(ax, ay, az), cell_origin=(0.0, 0.0, nabs * dz), unit_cells=cells,
+        vmin=-50.0, vmax=0.0,
+        packet=dict(x0=lx / 2, y0=ly / 2, z0=z0, sigma=1.8 * A * scale, kx=0.0, ky=0.0, kz=-k, amplitude=0.0),
+        k_det=k_det, every=20, steps=steps)
